@@ -1,0 +1,190 @@
+"""Seeded synthetic inputs for the mobility matvec (shared by tests, bench and oracle legs).
+
+This module holds geometry and random draws only -- none of the method's arithmetic
+(no RPY or wall formula appears here) -- so that the CUDA path and the CPU oracle can
+be fed the same inputs without sharing any code of the method itself.
+
+The five workloads are the ones ``BASELINE.json:configs`` names, made concrete in
+SURVEY.md 8(d) / DESIGN.md "Input recipe".  They stand in for the paper's own timing
+workload (rigid rods sedimented above a no-slip wall, a random force on every blob,
+PAPER.md:643), whose hard-rectangle packings are not available.
+
+Generator: ``numpy.random.default_rng(seed)`` (PCG64), float64, draws in the order
+written in each function; lengths in units of the blob radius a = 1, eta = 1; blob
+order is body-major.  The wall is z = 0 and the fluid occupies z > 0.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+
+@dataclass
+class Workload:
+    name: str
+    pos: np.ndarray            # [N,3] float64 blob positions
+    force: np.ndarray          # [k,N,3] float64 blob forces lambda
+    a: float = 1.0
+    eta: float = 1.0
+    blobs_per_body: int = 1
+    precisions: tuple = ("f64",)
+    variants: tuple = ("wall",)
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n_blobs(self) -> int:
+        return int(self.pos.shape[0])
+
+    @property
+    def n_rhs(self) -> int:
+        return int(self.force.shape[0])
+
+
+def quat_to_rot(q: np.ndarray) -> np.ndarray:
+    """Rotation matrices [nb,3,3] of unit quaternions q = (s, p1, p2, p3) [nb,4]."""
+    s, x, y, z = q[:, 0], q[:, 1], q[:, 2], q[:, 3]
+    R = np.empty((q.shape[0], 3, 3))
+    R[:, 0, 0] = 1 - 2 * (y * y + z * z); R[:, 0, 1] = 2 * (x * y - s * z); R[:, 0, 2] = 2 * (x * z + s * y)
+    R[:, 1, 0] = 2 * (x * y + s * z); R[:, 1, 1] = 1 - 2 * (x * x + z * z); R[:, 1, 2] = 2 * (y * z - s * x)
+    R[:, 2, 0] = 2 * (x * z - s * y); R[:, 2, 1] = 2 * (y * z + s * x); R[:, 2, 2] = 1 - 2 * (x * x + y * y)
+    return R
+
+
+def icosahedron_vertices() -> np.ndarray:
+    """The 12 vertices of a regular icosahedron on the unit sphere."""
+    phi = (1.0 + np.sqrt(5.0)) / 2.0
+    v = []
+    for s1 in (1.0, -1.0):
+        for s2 in (1.0, -1.0):
+            v.append((0.0, s1, s2 * phi))
+            v.append((s1, s2 * phi, 0.0))
+            v.append((s2 * phi, 0.0, s1))
+    v = np.array(v)
+    return v / np.linalg.norm(v, axis=1, keepdims=True)
+
+
+def shell_template(n_blobs: int = 42) -> np.ndarray:
+    """Unit-sphere shell of 12 or 42 blobs: icosahedron vertices, plus (42) the 30 edge
+    midpoints projected back to the sphere (one subdivision)."""
+    v = icosahedron_vertices()
+    if n_blobs == 12:
+        return v
+    if n_blobs != 42:
+        raise ValueError("shell_template: 12 or 42 blobs")
+    d = np.linalg.norm(v[:, None, :] - v[None, :, :], axis=2)
+    edge = d[d > 1e-9].min()
+    mids = []
+    for i in range(12):
+        for j in range(i + 1, 12):
+            if abs(d[i, j] - edge) < 1e-9:
+                m = 0.5 * (v[i] + v[j])
+                mids.append(m / np.linalg.norm(m))
+    mids = np.array(mids)
+    assert mids.shape == (30, 3)
+    return np.concatenate([v, mids], axis=0)
+
+
+def boomerang_template() -> np.ndarray:
+    """15-blob L shape: corner blob at the origin, two 7-blob arms along +x and +y,
+    blob spacing 2.1 a (BASELINE.json config 2; PAPER.md:750 defers the geometry to [68])."""
+    t = [(0.0, 0.0, 0.0)]
+    t += [(2.1 * m, 0.0, 0.0) for m in range(1, 8)]
+    t += [(0.0, 2.1 * m, 0.0) for m in range(1, 8)]
+    return np.array(t)
+
+
+def _forces(rng, k: int, n: int) -> np.ndarray:
+    return rng.standard_normal((k, n, 3))
+
+
+def config1(seed: int = 0, n: int = 2000, k: int = 1) -> Workload:
+    """Independent blobs in a box: x,y ~ U(0,60), z ~ U(1.2,20), then lambda ~ N(0,1)."""
+    rng = np.random.default_rng(seed)
+    x = rng.uniform(0.0, 60.0, n)
+    y = rng.uniform(0.0, 60.0, n)
+    z = rng.uniform(1.2, 20.0, n)
+    pos = np.stack([x, y, z], axis=1)
+    return Workload("cfg1_box2000" if n == 2000 else f"cfg1_box{n}", pos, _forces(rng, k, n),
+                    precisions=("f64",), meta={"seed": seed})
+
+
+def config2(seed: int = 0, n_bodies: int = 1000, k: int = 1) -> Workload:
+    """Boomerangs near the wall.  Draw order: quaternions N(0,1)[nb,4] (normalised),
+    centre x ~ U(0,400), y ~ U(0,400), z = |N(0, std 2)| + 2.5, then lambda.
+    The body 'centre' is the corner blob; every blob is then clamped to z >= 1.1."""
+    rng = np.random.default_rng(seed)
+    q = rng.standard_normal((n_bodies, 4))
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    cx = rng.uniform(0.0, 400.0, n_bodies)
+    cy = rng.uniform(0.0, 400.0, n_bodies)
+    cz = np.abs(rng.normal(0.0, 2.0, n_bodies)) + 2.5
+    tmpl = boomerang_template()
+    R = quat_to_rot(q)
+    pos = np.einsum("bij,tj->bti", R, tmpl) + np.stack([cx, cy, cz], axis=1)[:, None, :]
+    pos = pos.reshape(-1, 3)
+    pos[:, 2] = np.maximum(pos[:, 2], 1.1)
+    n = pos.shape[0]
+    return Workload(f"cfg2_boomerang{n}", pos, _forces(rng, k, n), blobs_per_body=15,
+                    precisions=("f64", "f32"), meta={"seed": seed, "n_bodies": n_bodies})
+
+
+def _shell_lattice(rng, side: int):
+    """side x side spheres of 42 blobs, shell radius 3, lattice spacing 8 with jitter
+    U(-0.5,0.5) in x and y, z ~ U(4.2,10); shells unrotated.  Draw order: jx, jy, z."""
+    nb = side * side
+    jx = rng.uniform(-0.5, 0.5, nb)
+    jy = rng.uniform(-0.5, 0.5, nb)
+    cz = rng.uniform(4.2, 10.0, nb)
+    ii, jj = np.meshgrid(np.arange(side), np.arange(side), indexing="ij")
+    cx = 8.0 * (ii.reshape(-1) + 0.5) + jx
+    cy = 8.0 * (jj.reshape(-1) + 0.5) + jy
+    tmpl = 3.0 * shell_template(42)
+    pos = tmpl[None, :, :] + np.stack([cx, cy, cz], axis=1)[:, None, :]
+    return pos.reshape(-1, 3)
+
+
+def config3(seed: int = 0, side: int = 64, k: int = 1) -> Workload:
+    """4,096 rigid 42-blob spheres = 172,032 blobs (side=64); then lambda."""
+    rng = np.random.default_rng(seed)
+    pos = _shell_lattice(rng, side)
+    n = pos.shape[0]
+    return Workload(f"cfg3_shells{n}", pos, _forces(rng, k, n), blobs_per_body=42,
+                    precisions=("f32", "f64"), meta={"seed": seed, "n_bodies": side * side})
+
+
+def config4(seed: int = 0, n: int = 1 << 20, k: int = 1) -> Workload:
+    """Dense sedimented monolayer: x,y ~ U(0,3000), z ~ U(1.1,5), then lambda."""
+    rng = np.random.default_rng(seed)
+    x = rng.uniform(0.0, 3000.0, n)
+    y = rng.uniform(0.0, 3000.0, n)
+    z = rng.uniform(1.1, 5.0, n)
+    pos = np.stack([x, y, z], axis=1)
+    return Workload(f"cfg4_monolayer{n}", pos, _forces(rng, k, n), precisions=("f32",),
+                    meta={"seed": seed})
+
+
+def config5(seed: int = 0, side: int = 64, k: int = 8) -> Workload:
+    """Geometry of config 3 with k = 8 simultaneous lambda vectors (same rng, forces drawn
+    after the geometry); run through the wall and the free-space kernels."""
+    rng = np.random.default_rng(seed)
+    pos = _shell_lattice(rng, side)
+    n = pos.shape[0]
+    return Workload(f"cfg5_shells{n}_k{k}", pos, _forces(rng, k, n), blobs_per_body=42,
+                    precisions=("f32",), variants=("wall", "free"),
+                    meta={"seed": seed, "n_bodies": side * side})
+
+
+CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+
+
+def make(config: int, **kw) -> Workload:
+    return CONFIGS[config](**kw)
+
+
+def sample_rows(n: int, n_rows: int, seed: int = 12345) -> np.ndarray:
+    """Seeded sorted sample of target rows used for parity / oracle timing at large N."""
+    if n_rows >= n:
+        return np.arange(n, dtype=np.int64)
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(n, size=n_rows, replace=False)).astype(np.int64)
