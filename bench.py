@@ -1,0 +1,412 @@
+#!/usr/bin/env python
+"""bench.py -- wall-RPY mobility matvec throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 1..5] [--prec f32|f64] [--variant wall|free] [--no-extra]
+
+A "step" is one pass of the whole hot path (prepack -> all-pairs -> finalise, i.e. one call of
+rpy_wall_matvec) over one synthetic workload.  Default workload: BASELINE.json configs[2]
+("config 3": 4,096 rigid 42-blob shells = 172,032 blobs, wall-corrected, fp32 path with fp64
+accumulation) -- the configuration north_star quotes its target on ("N >= 1.7e5 blobs").
+Prints ONE JSON line on stdout (rank 0); progress goes to stderr.
+
+Metric: G blob-pairs/s = N^2 / t / 1e9 (ordered pairs, i = j included; for k right-hand sides the
+pair-RHS products N^2 k / t are in "pair_rhs_gps").
+
+  value     device-resident inputs, CUDA-event time of K steps (L2 flushed between steps)
+  e2e       same metric through the C-ABI host-buffer call (pinned host tensors; H2D of
+            positions+forces and D2H of velocities inside the timed region)
+  roofline  ALU bound: algorithmic flops of the all-pairs kernel / its CUDA-event duration,
+            against 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (fp64: 64 lanes), DESIGN.md
+  cpu_baseline  the float64 oracle (oracle/) on this box's host cores, on a bounded row sample
+
+N > 1 (torchrun): target rows are sharded across ranks (each rank: its rows x all sources, no
+collective inside the data path), then one NCCL all-gather of u; strong scaling.
+--impl reference: times the oracle (this tier has no reference implementation to install).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "wall_rpy_matvec_blob_pairs_per_s"
+UNIT = "G blob-pairs/s"
+
+# Algorithmic work of the all-pairs kernel per ordered pair (recounted from
+# the SASS of the built kernels: FMA-pipe lane-instructions and flops with FMA = 2, MUL/ADD = 1).
+# k right-hand sides: geometry part + per-RHS apply part.
+WORK = {
+    # variant: (instr_geom, instr_per_rhs, flop_geom, flop_per_rhs)
+    "wall": (56, 10, 89, 18),
+    "free": (15, 10, 23, 18),
+}
+SM_COUNT = 148
+LANES = {"f32": 128, "f64": 64}
+SM_MAX_GHZ = 1.965
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def work_per_pair(variant: str, k: int):
+    ig, ir, fg, fr = WORK[variant]
+    return ig + ir * k, fg + fr * k
+
+
+def peak_tflops(prec: str) -> float:
+    return SM_COUNT * LANES[prec] * 2 * SM_MAX_GHZ * 1e9 / 1e12
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock, power and throttle reasons during the timed region (NVML)."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.sm_max, self.power = None, []
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # pragma: no cover
+            log(f"[bench] NVML unavailable: {e}")
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["unsampled"]}
+        s = sorted(self.samples)
+        load = [x for x in s if x >= 0.5 * s[-1]] or s
+        return {"sm_mhz": float(load[len(load) // 2]), "sm_max_mhz": float(self.sm_max or 0),
+                "reasons": sorted(self.reasons), "samples": len(s),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------------- oracle leg
+def oracle_sample(wl, variant: str, prec: str, budget_s: float, max_rows: int = 1 << 16):
+    """Times the oracle, as it stands, on a row sample sized for ~budget_s of CPU work.
+    Returns (G pairs/s, cores, description, seconds)."""
+    import oracle
+    from paper_1602_02170_b200 import workloads
+    ov = oracle.WALL if variant == "wall" else oracle.FREE
+    npdt = np.float32 if prec == "f32" else np.float64
+    pos = wl.pos.astype(npdt).astype(np.float64)
+    force = wl.force.astype(npdt).astype(np.float64)
+    n, k = wl.n_blobs, wl.n_rhs
+    cores = oracle.num_threads()
+    probe_rows = workloads.sample_rows(n, min(n, 4 * cores), seed=7)
+    t0 = time.perf_counter()
+    oracle.matvec(ov, pos, force, wl.a, wl.eta, rows=probe_rows)
+    t_probe = time.perf_counter() - t0
+    per_row = t_probe / len(probe_rows)
+    n_rows = int(max(cores, min(max_rows, n, budget_s / max(per_row, 1e-9))))
+    rows = workloads.sample_rows(n, n_rows, seed=12345)
+    t0 = time.perf_counter()
+    oracle.matvec(ov, pos, force, wl.a, wl.eta, rows=rows)
+    t = time.perf_counter() - t0
+    gps = len(rows) * n / t / 1e9
+    desc = f"{len(rows)} seeded target rows x all {n} sources, k={k}, {variant}, float64"
+    return gps, cores, desc, t, len(rows)
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1602_02170_b200 import workloads
+    wl = workloads.make(args.config)
+    k = wl.n_rhs
+    budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    times, rows_used, cores, desc = [], 0, 1, ""
+    for it in range(args.warmup + args.steps):
+        gps, cores, desc, t, nr = oracle_sample(wl, args.variant, args.prec, budget)
+        log(f"[reference] step {it}: {gps:.4f} {UNIT} ({t:.2f} s)")
+        if it >= args.warmup:
+            times.append(t); rows_used = nr
+    t_mean = float(np.mean(times))
+    value = rows_used * wl.n_blobs / t_mean / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_mean * 1e3,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": wl.name, "config_index": args.config, "n_blobs": wl.n_blobs, "n_rhs": k,
+                   "variant": args.variant, "step": "oracle on a bounded row sample: " + desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------- GPU leg
+def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, rank=0, world=1, dist=None):
+    """Device-resident timing of `steps` calls; returns dict with ms per step (max over ranks)."""
+    dt = torch.float32 if prec == "f32" else torch.float64
+    dev = torch.device("cuda", torch.cuda.current_device())
+    pos = torch.from_numpy(wl.pos).to(dt).to(dev)
+    force = torch.from_numpy(wl.force).to(dt).to(dev)
+    n, k = wl.n_blobs, wl.n_rhs
+    fn = binding.rpy_wall_matvec if variant == "wall" else binding.rpy_free_matvec
+    rb = rank * n // world
+    re_ = (rank + 1) * n // world
+    rows = None if world == 1 else (rb, re_ - rb)
+    ws = torch.empty(binding.rpy_matvec_workspace_bytes(prec, n, k), dtype=torch.uint8, device=dev)
+    out = torch.empty((k, n if rows is None else rows[1], 3), dtype=dt, device=dev)
+    gathered = None
+    if world > 1:
+        counts = [((r + 1) * n // world - r * n // world) for r in range(world)]
+        gathered = [torch.empty((k, c, 3), dtype=dt, device=dev) for c in counts]
+
+    def step():
+        fn(pos, force, wl.a, wl.eta, out=out, workspace=ws, rows=rows)
+        if world > 1:
+            dist.all_gather(gathered, out)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    evs = []
+    for _ in range(steps):
+        if flush_buf is not None:
+            flush_buf.zero_()                      # > L2 size: evicts the previous step's lines
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(); step(); e1.record()
+        evs.append((e0, e1))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in evs]
+    total = torch.tensor([sum(ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(total, op=dist.ReduceOp.MAX)
+    ms_per_step = total.item() / steps
+    return {"ms_per_step": ms_per_step, "ms_min": min(ms), "gps": n * n / (ms_per_step * 1e-3) / 1e9,
+            "pos": pos, "force": force, "ws": ws, "out": out if world == 1 else None}
+
+
+def time_allpairs_kernel(torch, binding, res, wl, variant, steps, flush_buf):
+    """CUDA events recorded by the library on its launch stream around the all-pairs kernel."""
+    times, pre, fin = [], [], []
+    for _ in range(steps):
+        if flush_buf is not None:
+            flush_buf.zero_()
+        _, ev = binding.rpy_matvec_phases(variant, res["pos"], res["force"], wl.a, wl.eta, out=res["out"],
+                                          workspace=res["ws"])
+        torch.cuda.synchronize()
+        pre.append(ev[0].elapsed_time(ev[1])); times.append(ev[1].elapsed_time(ev[2])); fin.append(ev[2].elapsed_time(ev[3]))
+    return float(np.mean(times)), float(np.mean(pre)), float(np.mean(fin))
+
+
+def time_e2e(torch, binding, wl, prec, variant, steps, warmup):
+    dt = torch.float32 if prec == "f32" else torch.float64
+    pos = torch.from_numpy(wl.pos).to(dt).pin_memory()
+    force = torch.from_numpy(wl.force).to(dt).pin_memory()
+    out = torch.empty(force.shape, dtype=dt).pin_memory()
+    n, k = wl.n_blobs, wl.n_rhs
+    dev = torch.device("cuda", torch.cuda.current_device())
+    scratch = torch.empty(binding.rpy_matvec_host_scratch_bytes(prec, n, k), dtype=torch.uint8, device=dev)
+    fn = binding.rpy_wall_matvec_host if variant == "wall" else binding.rpy_free_matvec_host
+    for _ in range(warmup):
+        fn(pos, force, wl.a, wl.eta, out=out, scratch=scratch)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        fn(pos, force, wl.a, wl.eta, out=out, scratch=scratch)      # synchronises before returning
+    t = (time.perf_counter() - t0) / steps
+    checksum = float(out.double().abs().sum())
+    es = 4 if prec == "f32" else 8
+    return {"value": n * n / t / 1e9, "unit": UNIT, "h2d_bytes_per_step": int((pos.numel() + force.numel()) * es),
+            "d2h_bytes_per_step": int(out.numel() * es), "ms_per_step": t * 1e3, "checksum_abs_u": checksum}
+
+
+def run_ours(args):
+    import torch
+    from paper_1602_02170_b200 import binding, workloads
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local % torch.cuda.device_count())
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", torch.cuda.current_device()))
+    binding.load_library()
+    dev = torch.device("cuda", torch.cuda.current_device())
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # 256 MiB > 126 MB L2
+
+    wl = workloads.make(args.config)
+    prec, variant = args.prec, args.variant
+    n, k = wl.n_blobs, wl.n_rhs
+    if rank == 0:
+        log(f"[bench] {wl.name}: N={n} k={k} {variant} {prec}, steps={args.steps} warmup={args.warmup} world={world}")
+
+    with ClockSampler(torch.cuda.current_device()) as clk:
+        res = time_config(torch, binding, wl, prec, variant, args.steps, args.warmup, flush, rank, world, dist)
+    clocks = clk.summary()
+    ms = res["ms_per_step"]
+    value = n * n / (ms * 1e-3) / 1e9
+    instr, flops = work_per_pair(variant, k)
+
+    line = None
+    if rank == 0:
+        # --- roofline of the dominant kernel (single-GPU geometry), timed on its own stream
+        if world == 1:
+            k_ms, pre_ms, fin_ms = time_allpairs_kernel(torch, binding, res, wl, variant, max(3, min(args.steps, 10)), flush)
+        else:
+            k_ms, pre_ms, fin_ms = ms, 0.0, 0.0
+        pairs_launch = (n // world if world > 1 else n) * n
+        achieved = pairs_launch * flops / (k_ms * 1e-3) / 1e12
+        peak = peak_tflops(prec)
+        # measured FMA-chain rate on this GPU, same run (context for the derived peak)
+        probe = {}
+        try:
+            for kind, name in ((0, "ffma"), (1, "ffma2"), (2, "dfma"), (3, "mufu_rsq")):
+                probe[name + "_g_per_s"] = round(binding.rpy_pipe_peak_probe(kind, 8192)["gfma_per_s"], 1)
+        except Exception as e:  # pragma: no cover
+            probe = {"error": str(e)}
+        lane_peak = SM_COUNT * LANES[prec] * SM_MAX_GHZ * 1e9
+        roofline = {
+            "bound": "alu", "kernel": "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "frac": achieved / peak, "traffic": None,
+            "peak_source": f"derived: {SM_COUNT} SM x {LANES[prec]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
+            "flop_per_pair": flops, "fma_pipe_instr_per_pair": instr,
+            "pipe_frac": pairs_launch * instr / (k_ms * 1e-3) / lane_peak,
+            "kernel_ms": k_ms, "prepack_ms": pre_ms, "finalise_ms": fin_ms,
+            "kernel_share_of_step": k_ms / (k_ms + pre_ms + fin_ms) if world == 1 else None,
+            "measured_chain_rates": probe,
+        }
+        # --- end to end through the host-buffer C-ABI call
+        e2e = time_e2e(torch, binding, wl, prec, variant, max(2, min(args.steps, 5)), 1) if world == 1 else \
+            {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+             "note": "host-buffer call is single-GPU; run with --gpus 1"}
+        # --- the oracle on the host cores, bounded sample
+        cpu = None
+        if world == 1 and not args.no_cpu:
+            gps, cores, desc, t, _ = oracle_sample(wl, variant, prec, 15.0)
+            cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
+        plan = binding.rpy_matvec_launch_plan(prec, n, k, n // world if world > 1 else n)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32 pair arithmetic, f64 accumulation" if prec == "f32" else "f64",
+            "data": "synthetic",
+            "config": {"workload": wl.name, "config_index": args.config, "n_blobs": n, "n_rhs": k,
+                       "variant": variant, "a": wl.a, "eta": wl.eta, "seed": wl.meta.get("seed"),
+                       "l2": "flushed between steps (256 MiB write)",
+                       "parallelism": "single GPU" if world == 1 else f"target rows sharded over {world} ranks + all-gather of u",
+                       "launch_plan": plan},
+            "pair_rhs_gps": value * k,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": 3 * args.steps * (1 if k <= 8 else -(-k // 8)),
+            "roofline": roofline, "cpu_baseline": cpu,
+        }
+        # --- the other BASELINE.json configurations, fewer steps (context; not the headline)
+        if world == 1 and not args.no_extra:
+            extra = []
+            for cfg, p, v, st in ((3, "f64", "wall", 3), (5, "f32", "wall", 3), (5, "f32", "free", 3),
+                                  (2, "f64", "wall", 10), (2, "f32", "wall", 10), (1, "f64", "wall", 10),
+                                  (4, "f32", "wall", 1)):
+                if (cfg, p, v) == (args.config, prec, variant):
+                    continue
+                w2 = workloads.make(cfg)
+                r2 = time_config(torch, binding, w2, p, v, st, 3 if cfg != 4 else 1, flush)
+                km, _, _ = time_allpairs_kernel(torch, binding, r2, w2, v, 2 if cfg != 4 else 1, flush)
+                i2, f2 = work_per_pair(v, w2.n_rhs)
+                lane2 = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
+                extra.append({"workload": w2.name, "prec": p, "variant": v, "n_blobs": w2.n_blobs, "n_rhs": w2.n_rhs,
+                              "ms_per_step": r2["ms_per_step"], "gps": r2["gps"], "pair_rhs_gps": r2["gps"] * w2.n_rhs,
+                              "kernel_ms": km,
+                              "pipe_frac": w2.n_blobs ** 2 * i2 / (km * 1e-3) / lane2,
+                              "flop_frac": w2.n_blobs ** 2 * f2 / (km * 1e-3) / 1e12 / peak_tflops(p)})
+                log(f"[bench] extra {extra[-1]}")
+                del r2
+            line["other_configs"] = extra
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--prec", choices=["f32", "f64"], default="f32")
+    ap.add_argument("--variant", choices=["wall", "free"], default="wall")
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configurations")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        log("[bench] note: fewer than 3 warm-up steps requested")
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

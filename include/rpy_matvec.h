@@ -1,0 +1,171 @@
+/*
+ * rpy_matvec.h -- C ABI of the B200-native RPY / wall-RPY blob mobility matvec.
+ *
+ * The operation (arXiv:1602.02170; line numbers are /root/reference/PAPER.md):
+ *
+ *   u_i = sum_{j=0}^{N-1} M_ij lambda_j        all j, including j = i      Eq. (6)
+ *
+ * evaluated by direct O(N_b^2) summation on one GPU, where the
+ * 3x3 block M_ij is
+ *
+ *   free space:  (1/(6 pi eta a)) RPY(r_i - r_j)                           Eq. (9)
+ *   single wall: the same plus the translation-translation Rotne-Prager-Blake wall
+ *                correction, i.e. Eq. (7) applied to the image part
+ *                of the half-space Green's function; closed form and the
+ *                readings taken where the paper is silent: DESIGN.md "Readings".
+ *
+ * The wall is the plane z = 0 (z is the third coordinate), the fluid is z > 0.  One
+ * radius `a` and one viscosity `eta` for all blobs.  The tensor is only meaningful for
+ * blob heights z >= a; heights are not checked by the matvec calls
+ * (rpy_wall_count_below is the optional O(N) check).  r <= 2a takes the overlap branch
+ * of Eq. (9); r = 0 (i = j or coincident blobs) gives M_ij = (6 pi eta a)^-1 I plus the
+ * wall term.
+ *
+ * Conventions common to every entry point
+ *  - "device" pointers are CUDA device pointers owned by the caller; "host" pointers
+ *    are ordinary host memory (pinned memory makes the host calls faster, it is not
+ *    required).  The library never allocates or frees memory and keeps no state between
+ *    calls except the thread-local last CUDA error code.
+ *  - Layouts (C order, densely packed): pos [n_blobs][3], force [n_rhs][n_blobs][3],
+ *    vel [n_rhs][n_blobs][3] (or [n_rhs][row_count][3] for the *_rows calls).  Element
+ *    type is double for RPY_PREC_F64 and float for RPY_PREC_F32_ACC64.  Blob order is
+ *    preserved.  vel is overwritten.  All pointers must be aligned to their element type.
+ *  - RPY_PREC_F64: every operation in IEEE double.  RPY_PREC_F32_ACC64: pair tensors in
+ *    float, partial sums over at most 128 sources in float, running sums in double,
+ *    output rounded to float once.
+ *  - Device calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*, NULL =
+ *    the legacy default stream) and return without synchronising.  The workspace must
+ *    stay untouched until that work has completed.
+ *  - Errors are return codes only.  Nothing is enqueued when a code other than RPY_OK or
+ *    RPY_ERR_CUDA is returned.  n_blobs == 0 (or row_count == 0) is RPY_OK and a no-op.
+ *  - All kernels are compiled for sm_100a only; on any other device the first launch
+ *    fails and RPY_ERR_CUDA is returned.  There is no CPU fallback.
+ */
+#ifndef RPY_MATVEC_H
+#define RPY_MATVEC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    RPY_OK = 0,
+    RPY_ERR_NULL = 1,       /* a required pointer is NULL                                   */
+    RPY_ERR_ARG = 2,        /* n_blobs < 0, n_rhs < 1, bad row range, a or eta not finite > 0,
+                               unknown precision, n_blobs above RPY_MAX_BLOBS               */
+    RPY_ERR_ALIAS = 3,      /* d_vel overlaps d_pos, d_force or the workspace               */
+    RPY_ERR_WORKSPACE = 4,  /* workspace smaller than rpy_matvec_workspace_bytes(), or not
+                               256-byte aligned                                             */
+    RPY_ERR_CUDA = 5        /* a CUDA runtime call failed; see rpy_last_cuda_error()        */
+} rpy_status;
+
+typedef enum {
+    RPY_PREC_F64 = 0,       /* double in, double arithmetic, double out                     */
+    RPY_PREC_F32_ACC64 = 1  /* float in, float pair arithmetic, double accumulation, float out */
+} rpy_prec;
+
+/* Largest n_blobs accepted (index arithmetic is 64-bit; the bound keeps N^2 work finite). */
+#define RPY_MAX_BLOBS ((int64_t)1 << 26)
+
+/* Bytes of device workspace the device calls need for (prec, n_blobs, n_rhs); 0 for
+ * n_blobs <= 0 or n_rhs < 1.  Holds the packed source records (PAPER.md:75 composite
+ * vectors r and lambda, rescaled by 1/a) and the double partial sums per source chunk.
+ * The same size serves the *_rows calls with any row range. */
+size_t rpy_matvec_workspace_bytes(rpy_prec prec, int64_t n_blobs, int n_rhs);
+
+/* u = M lambda with the wall-corrected tensor, all rows.
+ *   d_pos [n_blobs][3], d_force [n_rhs][n_blobs][3] : device, read only
+ *   d_vel [n_rhs][n_blobs][3]                        : device, overwritten
+ *   a, eta      : blob radius and viscosity, finite and > 0
+ *   d_workspace : device, 256-byte aligned, >= rpy_matvec_workspace_bytes() bytes          */
+rpy_status rpy_wall_matvec(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                           const void *d_pos, const void *d_force, void *d_vel,
+                           double a, double eta,
+                           void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* The same with the free-space RPY tensor, Eq. (9). */
+rpy_status rpy_free_matvec(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                           const void *d_pos, const void *d_force, void *d_vel,
+                           double a, double eta,
+                           void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Row-sharded forms: velocities of the target blobs row_begin .. row_begin+row_count-1
+ * only, summed over ALL n_blobs sources (rows of M are independent, PAPER.md:562
+ * "trivially parallelized"); this is the unit a multi-GPU caller gives each rank.
+ *   d_vel [n_rhs][row_count][3].   0 <= row_begin, row_begin + row_count <= n_blobs.   */
+rpy_status rpy_wall_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                                int64_t row_begin, int64_t row_count,
+                                const void *d_pos, const void *d_force, void *d_vel,
+                                double a, double eta,
+                                void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                                int64_t row_begin, int64_t row_count,
+                                const void *d_pos, const void *d_force, void *d_vel,
+                                double a, double eta,
+                                void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Host-buffer forms ("only the positions of the blobs need to be communicated",
+ * here positions and forces go up, velocities come back).
+ *   h_pos, h_force, h_vel : HOST pointers, layouts as above
+ *   d_scratch : device, 256-byte aligned, >= rpy_matvec_host_scratch_bytes() bytes
+ * Copies the inputs host->device on `cuda_stream`, runs the matvec, copies the result
+ * device->host and SYNCHRONISES the stream before returning, so h_vel is valid on return. */
+size_t rpy_matvec_host_scratch_bytes(rpy_prec prec, int64_t n_blobs, int n_rhs);
+rpy_status rpy_wall_matvec_host(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                                const void *h_pos, const void *h_force, void *h_vel,
+                                double a, double eta,
+                                void *d_scratch, size_t scratch_bytes, void *cuda_stream);
+rpy_status rpy_free_matvec_host(rpy_prec prec, int64_t n_blobs, int n_rhs,
+                                const void *h_pos, const void *h_force, void *h_vel,
+                                double a, double eta,
+                                void *d_scratch, size_t scratch_bytes, void *cuda_stream);
+
+/* Counts blobs with z < zmin (e.g. zmin = a: blobs overlapping the wall, for which the
+ * wall-corrected M is not positive definite).  d_count is a device
+ * int64 that is overwritten (zeroed, then accumulated) in stream order. */
+rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void *d_pos, double zmin,
+                                int64_t *d_count, void *cuda_stream);
+
+/* Measurement aid for the ALU roofline: runs a register-only chain
+ * of independent fused multiply-adds on every SM and writes the elapsed milliseconds
+ * (CUDA events on `cuda_stream`, which is synchronised) to *h_elapsed_ms and the number of
+ * scalar FMAs executed to *h_fma_count.  kind: 0 = FFMA (scalar float), 1 = packed
+ * fma.rn.f32x2 (two float FMAs per instruction), 2 = DFMA (double), 3 = MUFU.RSQ.
+ * d_sink: device buffer of at least 8 bytes (defeats dead-code elimination). */
+rpy_status rpy_pipe_peak_probe(int kind, int iters, void *d_sink, float *h_elapsed_ms,
+                               double *h_fma_count, void *cuda_stream);
+
+/* Measurement aid: the whole-matrix matvec (wall != 0: wall-corrected, else free space) with
+ * four caller-owned CUDA events (cudaEvent_t passed as void*) recorded on `cuda_stream`
+ *   [0] before prepack, [1] before the all-pairs kernel, [2] after it, [3] after finalise
+ * of the first right-hand-side group (n_rhs <= 8: the only one).  Same arguments, checks and
+ * result as rpy_wall_matvec / rpy_free_matvec otherwise; n_blobs >= 1.  bench.py uses it to
+ * time the dominant kernel on the stream it is launched on. */
+rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs,
+                             const void *d_pos, const void *d_force, void *d_vel,
+                             double a, double eta,
+                             void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                             void *const *cuda_events4);
+
+/* Launch geometry the all-pairs kernel would use for (prec, n_blobs, n_rhs, row_count):
+ * targets per CTA, number of source chunks, sources per shared-memory tile, CTAs.
+ * Pure host arithmetic (no CUDA call); any output pointer may be NULL. */
+rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_count,
+                                  int *targets_per_cta, int *n_source_chunks,
+                                  int *tile_sources, int64_t *n_ctas);
+
+const char *rpy_status_string(rpy_status s);
+
+/* cudaError_t (as int) of the last RPY_ERR_CUDA returned on the calling thread, else 0. */
+int rpy_last_cuda_error(void);
+
+/* Version of this ABI (bumped on any signature change). */
+int rpy_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RPY_MATVEC_H */

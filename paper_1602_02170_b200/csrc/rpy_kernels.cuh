@@ -1,0 +1,254 @@
+// rpy_kernels.cuh -- the three kernels of the hot path:
+//   prepack   O(N k): scale positions by 1/a and lay sources out as fixed-size records,
+//   allpairs  O(N^2 k): the direct sum of Eq. (6),
+//   finalise  O(N k): add the per-chunk double partials in fixed order, apply 1/(6 pi eta a).
+//
+// Source record ("group" = W consecutive sources, W = Lane::W):
+//   S x[W], y[W], z[W], then for every right-hand side  S lx[W], ly[W], lz[W],
+//   padded to a multiple of 16 bytes.  With W = 2 (packed float) one LDS.128 hands the
+//   inner loop x and y of two sources already in the register-pair form FFMA2 wants.
+// A staged tile is TILE_G consecutive records = one contiguous byte range, so it is
+// fetched with ONE 1-D bulk async copy (cp.async.bulk, TMA engine) completing on an
+// mbarrier; two buffers, the copy of tile t+1 overlaps the arithmetic on tile t.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "rpy_math.cuh"
+
+namespace rpy {
+
+template <class L, int K> struct RecLayout {
+    using S = typename L::S;
+    static constexpr int W = L::W;
+    static constexpr int PER16 = 16 / (int)sizeof(S);
+    static constexpr int RAW = (3 + 3 * K) * W;
+    static constexpr int LEN = (RAW + PER16 - 1) / PER16 * PER16;   // scalars per record
+    static constexpr int BYTES = LEN * (int)sizeof(S);
+};
+
+// ---------------------------------------------------------------------------- prepack
+// One thread per (padded) source.  Sources beyond n_blobs are padding: position (0,0,1),
+// zero force -- every coefficient stays finite and the contribution is exactly zero.
+template <class L, int K>
+__global__ void prepack_kernel(const typename L::S* __restrict__ pos,
+                               const typename L::S* __restrict__ force,   // [K][n][3] of this RHS group
+                               typename L::S* __restrict__ rec,
+                               int64_t n_blobs, int64_t n_padded, int64_t force_rhs_stride,
+                               double inv_a)
+{
+    using S = typename L::S;
+    using R = RecLayout<L, K>;
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_padded) return;
+    int64_t g = j / R::W;
+    int l = (int)(j % R::W);
+    S* r = rec + g * R::LEN;
+    bool real = j < n_blobs;
+    S x = real ? (S)((double)pos[3 * j + 0] * inv_a) : (S)0;
+    S y = real ? (S)((double)pos[3 * j + 1] * inv_a) : (S)0;
+    S z = real ? (S)((double)pos[3 * j + 2] * inv_a) : (S)1;
+    r[0 * R::W + l] = x;
+    r[1 * R::W + l] = y;
+    r[2 * R::W + l] = z;
+#pragma unroll
+    for (int s = 0; s < K; ++s) {
+        const S* f = force + (int64_t)s * force_rhs_stride + 3 * j;
+        r[(3 + 3 * s + 0) * R::W + l] = real ? f[0] : (S)0;
+        r[(3 + 3 * s + 1) * R::W + l] = real ? f[1] : (S)0;
+        r[(3 + 3 * s + 2) * R::W + l] = real ? f[2] : (S)0;
+    }
+    if (l == 0) {
+#pragma unroll
+        for (int q = R::RAW; q < R::LEN; ++q) r[q] = (S)0;
+    }
+}
+
+// ---------------------------------------------------------------------------- mbarrier / bulk copy
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk copy global -> shared (this CTA), completion counted in bytes on `bar`.
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------------------- all-pairs
+// Grid: x = target tile (BLOCK*T targets), y = source chunk.  Each thread keeps T targets in
+// registers (broadcast into every lane of V), walks the chunk's tiles from shared memory
+// (every lane of a warp reads the same record: a broadcast, no bank conflict), and keeps
+//   - float forms: per-target partial sums in V over FLUSH_G records (<= 128 sources), then
+//     adds them into double running sums (the "fp64 accumulation" of north_star);
+//   - double form: the running sums directly.
+// Output: partial[chunk][s][row][3] in double (row relative to row_begin).
+template <class L, int K, bool WALL, int T, int BLOCK, int TILE_G, int FLUSH_G, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+allpairs_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial,
+                int64_t row_begin, int64_t row_count, int64_t n_tiles, int tiles_per_chunk)
+{
+    using V = typename L::V;
+    using S = typename L::S;
+    using R = RecLayout<L, K>;
+    constexpr int W = L::W;
+    constexpr bool IS_F64 = sizeof(S) == 8;
+    constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
+    static_assert(TILE_G % FLUSH_G == 0, "flush period must divide the tile");
+    static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* const buf0 = smem_raw;      // buffer b lives at buf0 + b * TILE_BYTES
+    __shared__ __align__(8) uint64_t full_bar[2];
+
+    const int tid = threadIdx.x;
+    const int64_t tile_lo = (int64_t)blockIdx.y * tiles_per_chunk;
+    int64_t tile_hi = tile_lo + tiles_per_chunk;
+    if (tile_hi > n_tiles) tile_hi = n_tiles;
+    const int my_tiles = (int)(tile_hi - tile_lo);
+
+    if (tid == 0) {
+        mbar_init(&full_bar[0], 1);
+        mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const unsigned char* gsrc = reinterpret_cast<const unsigned char*>(rec) + tile_lo * (int64_t)TILE_BYTES;
+    if (tid == 0 && my_tiles > 0) {
+        mbar_expect_tx(&full_bar[0], TILE_BYTES);
+        bulk_g2s(buf0, gsrc, TILE_BYTES, &full_bar[0]);
+    }
+
+    // targets of this thread: rows row_begin + (blockIdx.x*BLOCK*T + t*BLOCK + tid); rows past
+    // the end recompute the last row and are not stored.
+    V xi[T], yi[T], zi[T];
+    int64_t row[T];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        row[t] = (int64_t)blockIdx.x * (BLOCK * T) + t * BLOCK + tid;
+        int64_t i = row_begin + (row[t] < row_count ? row[t] : row_count - 1);
+        const S* r = rec + (i / W) * R::LEN + (i % W);
+        xi[t] = L::bc((double)r[0 * W]);
+        yi[t] = L::bc((double)r[1 * W]);
+        zi[t] = L::bc((double)r[2 * W]);
+    }
+
+    double dacc[IS_F64 ? 1 : T][IS_F64 ? 1 : K][3];
+    V acc[T][K][3];
+#pragma unroll
+    for (int t = 0; t < T; ++t)
+#pragma unroll
+        for (int s = 0; s < K; ++s)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                acc[t][s][c] = L::bc(0.0);
+                if constexpr (!IS_F64) dacc[t][s][c] = 0.0;
+            }
+
+    for (int it = 0; it < my_tiles; ++it) {
+        const int b = it & 1;
+        // every thread is done with buffer b^1 (read in iteration it-1) before it is refilled
+        __syncthreads();
+        if (tid == 0 && it + 1 < my_tiles) {
+            mbar_expect_tx(&full_bar[b ^ 1], TILE_BYTES);
+            bulk_g2s(buf0 + (b ^ 1) * TILE_BYTES, gsrc + (int64_t)(it + 1) * TILE_BYTES, TILE_BYTES, &full_bar[b ^ 1]);
+        }
+        mbar_wait(&full_bar[b], (uint32_t)((it >> 1) & 1));
+        const S* tile = reinterpret_cast<const S*>(buf0 + b * TILE_BYTES);
+
+#pragma unroll 1
+        for (int g0 = 0; g0 < TILE_G; g0 += FLUSH_G) {
+#pragma unroll 2
+            for (int g = g0; g < g0 + FLUSH_G; ++g) {
+                const V* r = reinterpret_cast<const V*>(tile + g * R::LEN);
+                V xj = r[0], yj = r[1], zj = r[2];
+                V lam[K][3];
+#pragma unroll
+                for (int s = 0; s < K; ++s) {
+                    lam[s][0] = r[3 + 3 * s + 0];
+                    lam[s][1] = r[3 + 3 * s + 1];
+                    lam[s][2] = r[3 + 3 * s + 2];
+                }
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    PairCoef<V> c;
+                    pair_coef<L, WALL>(xi[t], yi[t], zi[t], xj, yj, zj, c);
+#pragma unroll
+                    for (int s = 0; s < K; ++s)
+                        pair_apply<L, WALL>(c, lam[s][0], lam[s][1], lam[s][2],
+                                            acc[t][s][0], acc[t][s][1], acc[t][s][2]);
+                }
+            }
+            if constexpr (!IS_F64) {
+#pragma unroll
+                for (int t = 0; t < T; ++t)
+#pragma unroll
+                    for (int s = 0; s < K; ++s)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            dacc[t][s][c] += L::hsum(acc[t][s][c]);
+                            acc[t][s][c] = L::bc(0.0);
+                        }
+            }
+        }
+    }
+
+    double* out = partial + (int64_t)blockIdx.y * K * row_count * 3;
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        if (row[t] < row_count) {
+#pragma unroll
+            for (int s = 0; s < K; ++s)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    if constexpr (IS_F64) out[((int64_t)s * row_count + row[t]) * 3 + c] = L::hsum(acc[t][s][c]);
+                    else                  out[((int64_t)s * row_count + row[t]) * 3 + c] = dacc[t][s][c];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------- finalise
+// vel[s][row][c] = scale * sum_{chunk} partial[chunk][s][row][c], chunks added in index order
+// (deterministic), one thread per output element.
+template <class S>
+__global__ void finalise_kernel(const double* __restrict__ partial, S* __restrict__ vel,
+                                int64_t per_chunk /* = K*row_count*3 */, int n_chunks,
+                                int64_t row_count3, int64_t vel_rhs_stride, double scale)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= per_chunk) return;
+    double sum = 0.0;
+    for (int c = 0; c < n_chunks; ++c) sum += partial[(int64_t)c * per_chunk + e];
+    int64_t s = e / row_count3, q = e % row_count3;
+    vel[s * vel_rhs_stride + q] = (S)(sum * scale);
+}
+
+template <class S>
+__global__ void count_below_kernel(const S* __restrict__ pos, int64_t n, double zmin,
+                                   unsigned long long* __restrict__ count)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool below = i < n && (double)pos[3 * i + 2] < zmin;
+    unsigned m = __ballot_sync(0xffffffffu, below);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, (unsigned long long)__popc(m));
+}
+
+}  // namespace rpy

@@ -1,0 +1,394 @@
+// rpy_matvec.cu -- host side of the C ABI declared in include/rpy_matvec.h: argument checks,
+// launch planning, and the prepack -> all-pairs -> finalise launch sequence.  No allocation,
+// no synchronisation (except the *_host forms), no state.  sm_100a only.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/rpy_matvec.h"
+#include "rpy_kernels.cuh"
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+constexpr int kAbiVersion = 1;
+constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
+constexpr int kTargetCtas = kNumSMs * 16;  // CTAs wanted before sources are no longer chunked
+constexpr int kMaxChunks = 64;
+constexpr int kBlock = 128;
+constexpr int kMaxT = 2;
+constexpr size_t kAlign = 256;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Per (precision, K) kernel shape.  TILE_G records per staged tile, FLUSH_G records per
+// float->double flush (W*FLUSH_G <= 128 sources, the bound stated in the header).
+template <class L, int K> struct Shape;
+template <int K> struct Shape<rpy::Lane<float2>, K> {
+    static constexpr int TILE_G = 64, FLUSH_G = 64, MINB = (K >= 4 ? 2 : 4);
+};
+template <int K> struct Shape<rpy::Lane<double>, K> {
+    static constexpr int TILE_G = 64, FLUSH_G = 64, MINB = (K >= 4 ? 1 : 2);
+};
+
+struct Plan {
+    int T;                 // targets per thread
+    int targets_per_cta;
+    int tile_sources;      // W * TILE_G
+    int64_t n_padded;      // sources incl. padding
+    int64_t n_tiles;
+    int tiles_per_chunk;
+    int n_chunks;
+    int64_t n_target_tiles;
+};
+
+inline int tile_sources_of(rpy_prec prec) { return prec == RPY_PREC_F64 ? 64 : 128; }
+inline size_t elem_size(rpy_prec prec) { return prec == RPY_PREC_F64 ? 8 : 4; }
+
+// scalars per record, mirrors rpy::RecLayout
+inline size_t record_bytes(rpy_prec prec, int K)
+{
+    int W = prec == RPY_PREC_F64 ? 1 : 2;
+    int per16 = 16 / (int)elem_size(prec);
+    int raw = (3 + 3 * K) * W;
+    return (size_t)((raw + per16 - 1) / per16 * per16) * elem_size(prec);
+}
+
+Plan make_plan(rpy_prec prec, int64_t n, int K, int64_t rows)
+{
+    Plan p;
+    p.tile_sources = tile_sources_of(prec);
+    p.n_padded = (n + p.tile_sources - 1) / p.tile_sources * p.tile_sources;
+    p.n_tiles = p.n_padded / p.tile_sources;
+    // two targets per thread once there are enough rows to fill the chip that way
+    // (K >= 4 already holds 3K accumulators per target: one target per thread there)
+    p.T = (K <= 2 && rows >= (int64_t)kNumSMs * kBlock * 2 * 2) ? 2 : 1;
+    p.targets_per_cta = kBlock * p.T;
+    p.n_target_tiles = (rows + p.targets_per_cta - 1) / p.targets_per_cta;
+    int64_t want = p.n_target_tiles > 0 ? (kTargetCtas + p.n_target_tiles - 1) / p.n_target_tiles : 1;
+    if (want > kMaxChunks) want = kMaxChunks;
+    if (want > p.n_tiles) want = p.n_tiles;
+    if (want < 1) want = 1;
+    p.tiles_per_chunk = (int)((p.n_tiles + want - 1) / want);
+    if (p.tiles_per_chunk < 1) p.tiles_per_chunk = 1;
+    p.n_chunks = (int)((p.n_tiles + p.tiles_per_chunk - 1) / p.tiles_per_chunk);
+    if (p.n_chunks < 1) p.n_chunks = 1;
+    return p;
+}
+
+inline int group_k(int remaining) { return remaining >= 8 ? 8 : remaining >= 4 ? 4 : remaining >= 2 ? 2 : 1; }
+
+size_t records_bytes(rpy_prec prec, int64_t n, int K)
+{
+    int ts = tile_sources_of(prec);
+    int64_t n_padded = (n + ts - 1) / ts * ts;
+    int W = prec == RPY_PREC_F64 ? 1 : 2;
+    return align_up((size_t)(n_padded / W) * record_bytes(prec, K), kAlign);
+}
+
+// n_chunks * rows <= kTargetCtas * kBlock * kMaxT + rows  (n_chunks <= kTargetCtas / n_target_tiles + 1)
+size_t partial_bytes_bound(int64_t n, int K)
+{
+    return align_up((size_t)((int64_t)kTargetCtas * kBlock * kMaxT + n) * (size_t)K * 3 * sizeof(double), kAlign);
+}
+
+size_t workspace_bytes(rpy_prec prec, int64_t n, int n_rhs)
+{
+    if (n <= 0 || n_rhs < 1) return 0;
+    int K = group_k(n_rhs);
+    return records_bytes(prec, n, K) + partial_bytes_bound(n, K);
+}
+
+inline rpy_status cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    return RPY_ERR_CUDA;
+}
+
+inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn)
+{
+    uintptr_t a = (uintptr_t)p, b = (uintptr_t)q;
+    return pn && qn && a < b + qn && b < a + pn;
+}
+
+template <class L, int K, bool WALL, int T>
+cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, double* partial,
+                            int64_t row_begin, int64_t rows, cudaStream_t st)
+{
+    using Sh = Shape<L, K>;
+    constexpr int TILE_G = Sh::TILE_G;
+    auto kern = rpy::allpairs_kernel<L, K, WALL, T, kBlock, TILE_G, Sh::FLUSH_G, Sh::MINB>;
+    size_t smem = 2 * (size_t)TILE_G * rpy::RecLayout<L, K>::BYTES;
+    dim3 grid((unsigned)p.n_target_tiles, (unsigned)p.n_chunks);
+    kern<<<grid, kBlock, smem, st>>>(rec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
+    return cudaGetLastError();
+}
+
+template <class L, int K>
+cudaError_t run_group(bool wall, const Plan& p, int64_t n, int64_t row_begin, int64_t rows,
+                      const typename L::S* pos, const typename L::S* force, typename L::S* vel,
+                      double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev)
+{
+    using S = typename L::S;
+    S* rec = reinterpret_cast<S*>(ws);
+    rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
+    double* partial = reinterpret_cast<double*>(ws + records_bytes(prec, n, K));
+    {
+        int threads = 256;
+        int64_t blocks = (p.n_padded + threads - 1) / threads;
+        rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, p.n_padded,
+                                                                      n * 3, 1.0 / a);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    cudaError_t e;
+    if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
+    constexpr int T2 = K <= 2 ? 2 : 1;     // make_plan never asks for T = 2 when K > 2
+    if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, partial, row_begin, rows, st)
+                           : launch_allpairs<L, K, true, 1>(p, rec, partial, row_begin, rows, st);
+    else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, partial, row_begin, rows, st)
+                           : launch_allpairs<L, K, false, 1>(p, rec, partial, row_begin, rows, st);
+    if (e != cudaSuccess) return e;
+    if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[2]), st)) != cudaSuccess) return e;
+    {
+        int64_t per_chunk = (int64_t)K * rows * 3;
+        int threads = 256;
+        int64_t blocks = (per_chunk + threads - 1) / threads;
+        const double PI = 3.14159265358979323846;
+        rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, vel, per_chunk, p.n_chunks,
+                                                                    rows * 3, rows * 3,
+                                                                    1.0 / (6.0 * PI * eta * a));
+        e = cudaGetLastError();
+    }
+    return e;
+}
+
+template <class L>
+cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
+                           const void* d_pos, const void* d_force, void* d_vel,
+                           double a, double eta, void* ws, cudaStream_t st, void* const* ev)
+{
+    using S = typename L::S;
+    rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
+    cudaError_t ee;
+    if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[0]), st)) != cudaSuccess) return ee;
+    const S* pos = static_cast<const S*>(d_pos);
+    int done = 0;
+    while (done < n_rhs) {
+        int K = group_k(n_rhs - done);
+        const S* force = static_cast<const S*>(d_force) + (int64_t)done * n * 3;
+        S* vel = static_cast<S*>(d_vel) + (int64_t)done * rows * 3;
+        unsigned char* w = static_cast<unsigned char*>(ws);
+        Plan p = make_plan(prec, n, K, rows);
+        cudaError_t e;
+        switch (K) {
+            case 8: e = run_group<L, 8>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 4: e = run_group<L, 4>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 2: e = run_group<L, 2>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            default: e = run_group<L, 1>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+        }
+        if (e != cudaSuccess) return e;
+        done += K;
+    }
+    if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[3]), st)) != cudaSuccess) return ee;
+    return cudaSuccess;
+}
+
+rpy_status matvec_rows(bool wall, rpy_prec prec, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
+                       const void* d_pos, const void* d_force, void* d_vel, double a, double eta,
+                       void* ws, size_t ws_bytes, void* stream, void* const* ev = nullptr)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n < 0 || n > RPY_MAX_BLOBS || n_rhs < 1) return RPY_ERR_ARG;
+    if (row_begin < 0 || rows < 0 || row_begin > n || rows > n - row_begin) return RPY_ERR_ARG;
+    if (!(a > 0.0) || !(eta > 0.0) || !isfinite(a) || !isfinite(eta)) return RPY_ERR_ARG;
+    if (n == 0 || rows == 0) return RPY_OK;
+    if (!d_pos || !d_force || !d_vel || !ws) return RPY_ERR_NULL;
+    size_t es = elem_size(prec);
+    size_t pos_b = (size_t)n * 3 * es, force_b = pos_b * (size_t)n_rhs, vel_b = (size_t)rows * 3 * es * (size_t)n_rhs;
+    size_t need = workspace_bytes(prec, n, n_rhs);
+    if (ws_bytes < need || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    if (overlaps(d_vel, vel_b, d_pos, pos_b) || overlaps(d_vel, vel_b, d_force, force_b) ||
+        overlaps(d_vel, vel_b, ws, need))
+        return RPY_ERR_ALIAS;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = prec == RPY_PREC_F64
+        ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev)
+        : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
+
+size_t host_scratch_bytes(rpy_prec prec, int64_t n, int n_rhs)
+{
+    if (n <= 0 || n_rhs < 1) return 0;
+    size_t es = elem_size(prec);
+    size_t pos_b = align_up((size_t)n * 3 * es, kAlign);
+    size_t f_b = align_up((size_t)n * 3 * es * (size_t)n_rhs, kAlign);
+    return pos_b + 2 * f_b + workspace_bytes(prec, n, n_rhs);
+}
+
+rpy_status matvec_host(bool wall, rpy_prec prec, int64_t n, int n_rhs, const void* h_pos, const void* h_force,
+                       void* h_vel, double a, double eta, void* d_scratch, size_t scratch_bytes, void* stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n < 0 || n > RPY_MAX_BLOBS || n_rhs < 1) return RPY_ERR_ARG;
+    if (!(a > 0.0) || !(eta > 0.0) || !isfinite(a) || !isfinite(eta)) return RPY_ERR_ARG;
+    if (n == 0) return RPY_OK;
+    if (!h_pos || !h_force || !h_vel || !d_scratch) return RPY_ERR_NULL;
+    if (scratch_bytes < host_scratch_bytes(prec, n, n_rhs) || ((uintptr_t)d_scratch % kAlign) != 0)
+        return RPY_ERR_WORKSPACE;
+    size_t es = elem_size(prec);
+    size_t pos_raw = (size_t)n * 3 * es, f_raw = pos_raw * (size_t)n_rhs;
+    size_t pos_b = align_up(pos_raw, kAlign), f_b = align_up(f_raw, kAlign);
+    unsigned char* base = static_cast<unsigned char*>(d_scratch);
+    void* d_pos = base;
+    void* d_force = base + pos_b;
+    void* d_vel = base + pos_b + f_b;
+    void* ws = base + pos_b + 2 * f_b;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaMemcpyAsync(d_pos, h_pos, pos_raw, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaMemcpyAsync(d_force, h_force, f_raw, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    rpy_status s = matvec_rows(wall, prec, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws,
+                               workspace_bytes(prec, n, n_rhs), stream);
+    if (s != RPY_OK) return s;
+    e = cudaMemcpyAsync(h_vel, d_vel, f_raw, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t rpy_matvec_workspace_bytes(rpy_prec prec, int64_t n_blobs, int n_rhs)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return 0;
+    if (n_blobs > RPY_MAX_BLOBS) return 0;
+    return workspace_bytes(prec, n_blobs, n_rhs);
+}
+
+rpy_status rpy_wall_matvec(rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos, const void* d_force,
+                           void* d_vel, double a, double eta, void* d_workspace, size_t workspace_bytes_,
+                           void* cuda_stream)
+{
+    return matvec_rows(true, prec, n_blobs, n_rhs, 0, n_blobs < 0 ? 0 : n_blobs, d_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_free_matvec(rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos, const void* d_force,
+                           void* d_vel, double a, double eta, void* d_workspace, size_t workspace_bytes_,
+                           void* cuda_stream)
+{
+    return matvec_rows(false, prec, n_blobs, n_rhs, 0, n_blobs < 0 ? 0 : n_blobs, d_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_wall_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_begin, int64_t row_count,
+                                const void* d_pos, const void* d_force, void* d_vel, double a, double eta,
+                                void* d_workspace, size_t workspace_bytes_, void* cuda_stream)
+{
+    if (n_blobs < 0) return RPY_ERR_ARG;
+    return matvec_rows(true, prec, n_blobs, n_rhs, row_begin, row_count, d_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_begin, int64_t row_count,
+                                const void* d_pos, const void* d_force, void* d_vel, double a, double eta,
+                                void* d_workspace, size_t workspace_bytes_, void* cuda_stream)
+{
+    if (n_blobs < 0) return RPY_ERR_ARG;
+    return matvec_rows(false, prec, n_blobs, n_rhs, row_begin, row_count, d_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos,
+                             const void* d_force, void* d_vel, double a, double eta, void* d_workspace,
+                             size_t workspace_bytes_, void* cuda_stream, void* const* cuda_events4)
+{
+    if (!cuda_events4 || !cuda_events4[0] || !cuda_events4[1] || !cuda_events4[2] || !cuda_events4[3])
+        return RPY_ERR_NULL;
+    if (n_blobs < 1) return RPY_ERR_ARG;
+    return matvec_rows(wall != 0, prec, n_blobs, n_rhs, 0, n_blobs, d_pos, d_force, d_vel, a, eta, d_workspace,
+                       workspace_bytes_, cuda_stream, cuda_events4);
+}
+
+size_t rpy_matvec_host_scratch_bytes(rpy_prec prec, int64_t n_blobs, int n_rhs)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return 0;
+    if (n_blobs > RPY_MAX_BLOBS) return 0;
+    return host_scratch_bytes(prec, n_blobs, n_rhs);
+}
+
+rpy_status rpy_wall_matvec_host(rpy_prec prec, int64_t n_blobs, int n_rhs, const void* h_pos, const void* h_force,
+                                void* h_vel, double a, double eta, void* d_scratch, size_t scratch_bytes,
+                                void* cuda_stream)
+{
+    return matvec_host(true, prec, n_blobs, n_rhs, h_pos, h_force, h_vel, a, eta, d_scratch, scratch_bytes, cuda_stream);
+}
+
+rpy_status rpy_free_matvec_host(rpy_prec prec, int64_t n_blobs, int n_rhs, const void* h_pos, const void* h_force,
+                                void* h_vel, double a, double eta, void* d_scratch, size_t scratch_bytes,
+                                void* cuda_stream)
+{
+    return matvec_host(false, prec, n_blobs, n_rhs, h_pos, h_force, h_vel, a, eta, d_scratch, scratch_bytes, cuda_stream);
+}
+
+rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void* d_pos, double zmin, int64_t* d_count,
+                                void* cuda_stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n_blobs < 0 || n_blobs > RPY_MAX_BLOBS || isnan(zmin)) return RPY_ERR_ARG;
+    if (!d_count) return RPY_ERR_NULL;
+    if (n_blobs > 0 && !d_pos) return RPY_ERR_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = cudaMemsetAsync(d_count, 0, sizeof(int64_t), st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (n_blobs == 0) return RPY_OK;
+    int threads = 256;
+    unsigned blocks = (unsigned)((n_blobs + threads - 1) / threads);
+    auto* cnt = reinterpret_cast<unsigned long long*>(d_count);
+    if (prec == RPY_PREC_F64)
+        rpy::count_below_kernel<double><<<blocks, threads, 0, st>>>(static_cast<const double*>(d_pos), n_blobs, zmin, cnt);
+    else
+        rpy::count_below_kernel<float><<<blocks, threads, 0, st>>>(static_cast<const float*>(d_pos), n_blobs, zmin, cnt);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
+
+rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_count,
+                                  int* targets_per_cta, int* n_source_chunks, int* tile_sources, int64_t* n_ctas)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n_blobs < 0 || n_blobs > RPY_MAX_BLOBS || n_rhs < 1 || row_count < 0 || row_count > n_blobs) return RPY_ERR_ARG;
+    Plan p = make_plan(prec, n_blobs, group_k(n_rhs), row_count);
+    if (targets_per_cta) *targets_per_cta = p.targets_per_cta;
+    if (n_source_chunks) *n_source_chunks = p.n_chunks;
+    if (tile_sources) *tile_sources = p.tile_sources;
+    if (n_ctas) *n_ctas = p.n_target_tiles * p.n_chunks;
+    return RPY_OK;
+}
+
+const char* rpy_status_string(rpy_status s)
+{
+    switch (s) {
+        case RPY_OK: return "RPY_OK";
+        case RPY_ERR_NULL: return "RPY_ERR_NULL: a required pointer is NULL";
+        case RPY_ERR_ARG: return "RPY_ERR_ARG: invalid size, range, precision, radius or viscosity";
+        case RPY_ERR_ALIAS: return "RPY_ERR_ALIAS: output overlaps an input or the workspace";
+        case RPY_ERR_WORKSPACE: return "RPY_ERR_WORKSPACE: workspace too small or misaligned";
+        case RPY_ERR_CUDA: return "RPY_ERR_CUDA: a CUDA runtime call failed (rpy_last_cuda_error)";
+    }
+    return "unknown rpy_status";
+}
+
+int rpy_last_cuda_error(void) { return g_last_cuda_error; }
+int rpy_abi_version(void) { return kAbiVersion; }
+
+}  // extern "C"

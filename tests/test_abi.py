@@ -1,0 +1,162 @@
+"""Host-side checks of the C ABI that need no GPU: the library builds and loads, exports every
+symbol include/rpy_matvec.h declares, validates arguments before touching CUDA, and its launch
+planning / workspace arithmetic is consistent."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_1602_02170_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "rpy_matvec.h")
+
+F64, F32 = binding.RPY_PREC_F64, binding.RPY_PREC_F32_ACC64
+
+
+def _declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(rpy_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    lib = binding.load_library()
+    names = _declared_symbols()
+    assert "rpy_wall_matvec" in names and "rpy_free_matvec" in names and len(names) >= 14
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in the header but not exported"
+    assert set(names) == set(binding.SIGNATURES), "binding and header disagree on the symbol list"
+    assert lib.rpy_abi_version() == 1
+
+
+def test_no_torch_or_oracle_in_native_symbols():
+    # the boundary is plain C: no C++-mangled torch symbols are needed to load it
+    out = os.popen(f"nm -D --undefined-only {binding.library_path()}").read()
+    assert "c10" not in out and "at::" not in out and "torch" not in out
+    assert "rpy_oracle" not in out
+
+
+def test_status_strings():
+    for code, name in [(0, "RPY_OK"), (1, "RPY_ERR_NULL"), (2, "RPY_ERR_ARG"), (3, "RPY_ERR_ALIAS"),
+                       (4, "RPY_ERR_WORKSPACE"), (5, "RPY_ERR_CUDA")]:
+        assert binding.rpy_status_string(code).startswith(name)
+    assert "unknown" in binding.rpy_status_string(99)
+
+
+def test_workspace_bytes_monotone_and_zero_cases():
+    w = binding.rpy_matvec_workspace_bytes
+    assert w(F64, 0, 1) == 0 and w(F32, -5, 1) == 0 and w(F64, 100, 0) == 0
+    for prec in (F64, F32):
+        prev = 0
+        for n in (1, 127, 128, 129, 2000, 15000, 172032, 1 << 20):
+            b = w(prec, n, 1)
+            assert b >= prev and b % 256 == 0 and b > 0
+            prev = b
+        assert w(prec, 2000, 8) > w(prec, 2000, 1)
+        # n_rhs = 11 is processed as groups 8 + 2 + 1: the largest group sizes the workspace
+        assert w(prec, 2000, 11) == w(prec, 2000, 8)
+    # fp32 records are half the size of fp64 ones
+    assert w(F32, 1 << 20, 1) < w(F64, 1 << 20, 1)
+    # host scratch = inputs + output + workspace
+    h = binding.rpy_matvec_host_scratch_bytes
+    assert h(F64, 1000, 2) >= w(F64, 1000, 2) + 3 * 1000 * 3 * 8
+    assert h(F32, 0, 1) == 0
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("n,k", [(2000, 1), (15000, 1), (172032, 1), (1 << 20, 1), (172032, 8), (1, 1), (129, 3)])
+def test_launch_plan_covers_all_sources_and_fits_workspace(prec, n, k):
+    for rows in sorted({n, max(1, n // 2), 1}):
+        p = binding.rpy_matvec_launch_plan(prec, n, k, rows)
+        ts, tpc, nch = p["tile_sources"], p["targets_per_cta"], p["n_source_chunks"]
+        n_tiles = -(-n // ts)
+        assert 1 <= nch <= max(1, n_tiles)
+        tiles_per_chunk = -(-n_tiles // nch)
+        assert tiles_per_chunk * nch >= n_tiles                 # every tile is in some chunk
+        assert tiles_per_chunk * (nch - 1) < n_tiles            # no empty chunk
+        assert p["n_ctas"] == -(-rows // tpc) * nch
+        # partial sums [chunk][k][rows][3] doubles + packed records fit the advertised workspace
+        kg = 8 if k >= 8 else 4 if k >= 4 else 2 if k >= 2 else 1
+        w = 2 if prec == F32 else 1
+        es = 4 if prec == F32 else 8
+        rec = -(-((3 + 3 * kg) * w * es) // 16) * 16
+        need = (-(-n // ts) * ts // w) * rec + nch * kg * rows * 3 * 8
+        assert need <= binding.rpy_matvec_workspace_bytes(prec, n, k)
+    if n >= 172032 and k == 1:
+        assert p is not None
+        full = binding.rpy_matvec_launch_plan(prec, n, k, n)
+        assert full["n_ctas"] >= 148 * 4      # enough CTAs for several waves on 148 SMs
+
+
+def test_argument_errors_are_returned_before_any_cuda_work():
+    lib = binding.load_library()
+    one = ctypes.create_string_buffer(4096)
+    p = ctypes.addressof(one)
+
+    def call(prec=F64, n=4, k=1, pos=p, force=p + 1024, vel=p + 2048, a=1.0, eta=1.0, ws=p, wsb=0, fn="rpy_wall_matvec"):
+        return getattr(lib, fn)(prec, n, k, pos, force, vel, a, eta, ws, wsb, None)
+
+    for fn in ("rpy_wall_matvec", "rpy_free_matvec", "rpy_wall_matvec_host", "rpy_free_matvec_host"):
+        assert call(n=-1, fn=fn) == 2
+        assert call(k=0, fn=fn) == 2
+        assert call(prec=7, fn=fn) == 2
+        assert call(a=0.0, fn=fn) == 2 and call(a=-1.0, fn=fn) == 2 and call(a=float("nan"), fn=fn) == 2
+        assert call(eta=0.0, fn=fn) == 2 and call(eta=float("inf"), fn=fn) == 2
+        assert call(n=0, fn=fn) == 0                              # empty problem: OK, no-op
+        assert call(pos=None, fn=fn) == 1 and call(force=None, fn=fn) == 1 and call(vel=None, fn=fn) == 1
+        assert call(ws=None, fn=fn) == 1
+        assert call(wsb=16, fn=fn) == 4                           # workspace too small
+    assert call(n=(1 << 26) + 1) == 2
+    big = binding.rpy_matvec_workspace_bytes(F64, 4, 1)
+    aligned = (p + 255) // 256 * 256
+    # misaligned workspace, then aliasing output
+    assert call(ws=aligned + 8, wsb=big) == 4
+    assert call(ws=aligned, wsb=big, vel=p, pos=p) == 3
+    assert call(ws=aligned, wsb=big, vel=p + 1024 + 8, force=p + 1024) == 3
+    # row ranges
+    rows = lib.rpy_wall_matvec_rows
+    assert rows(F64, 4, 1, -1, 2, p, p, p, 1.0, 1.0, p, 0, None) == 2
+    assert rows(F64, 4, 1, 3, 2, p, p, p, 1.0, 1.0, p, 0, None) == 2
+    assert rows(F64, 4, 1, 2, 0, p, p, p, 1.0, 1.0, p, 0, None) == 0
+    assert lib.rpy_free_matvec_rows(F64, -4, 1, 0, 0, p, p, p, 1.0, 1.0, p, 0, None) == 2
+    # count_below / probe / plan argument checks
+    assert lib.rpy_wall_count_below(F64, -1, p, 1.0, p, None) == 2
+    assert lib.rpy_wall_count_below(F64, 4, p, 1.0, None, None) == 1
+    assert lib.rpy_pipe_peak_probe(9, 10, p, None, None, None) == 2
+    assert lib.rpy_pipe_peak_probe(0, 10, None, None, None, None) == 1
+    assert lib.rpy_matvec_launch_plan(F64, 10, 1, 11, None, None, None, None) == 2
+    assert lib.rpy_last_cuda_error() == 0
+
+
+def test_python_binding_refuses_cpu_tensors_and_bad_shapes():
+    import torch
+    pos = torch.zeros(4, 3, dtype=torch.float64)
+    lam = torch.zeros(4, 3, dtype=torch.float64)
+    with pytest.raises((RuntimeError, ValueError)):
+        binding.rpy_wall_matvec(pos, lam)            # no CUDA / CPU tensor: no fallback
+    with pytest.raises((RuntimeError, ValueError)):
+        binding.rpy_free_matvec(pos, lam)
+    with pytest.raises(TypeError):
+        binding._prec_of(torch.float16)
+    with pytest.raises(ValueError):
+        binding._shape_inputs(torch.zeros(4, 2), lam)
+    with pytest.raises(ValueError):
+        binding._shape_inputs(pos, torch.zeros(2, 5, 3, dtype=torch.float64))
+    with pytest.raises(TypeError):
+        binding._shape_inputs(pos, torch.zeros(4, 3, dtype=torch.float32))
+    assert binding._shape_inputs(pos, torch.zeros(2, 4, 3, dtype=torch.float64)) == (4, 2, False)
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1602_02170_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "rpy_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_1602_02170_b200 import" not in txt and "import paper_1602_02170_b200" not in txt
