@@ -133,7 +133,9 @@ rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void *d_po
  * of independent fused multiply-adds on every SM and writes the elapsed milliseconds
  * (CUDA events on `cuda_stream`, which is synchronised) to *h_elapsed_ms and the number of
  * scalar FMAs executed to *h_fma_count.  kind: 0 = FFMA (scalar float), 1 = packed
- * fma.rn.f32x2 (two float FMAs per instruction), 2 = DFMA (double), 3 = MUFU.RSQ.
+ * fma.rn.f32x2 (two float FMAs per instruction), 2 = DFMA (double), 3 = MUFU.RSQ,
+ * 4 = packed f32x2 with three distinct register-pair operands, 5 = FFMA with three distinct
+ * register operands (kinds 0-2 multiply by loop-invariant registers).
  * d_sink: device buffer of at least 8 bytes (defeats dead-code elimination). */
 rpy_status rpy_pipe_peak_probe(int kind, int iters, void *d_sink, float *h_elapsed_ms,
                                double *h_fma_count, void *cuda_stream);

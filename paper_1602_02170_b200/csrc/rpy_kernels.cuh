@@ -187,13 +187,31 @@ allpairs_kernel(const typename L::S* __restrict__ rec, double* __restrict__ part
                     lam[s][1] = r[3 + 3 * s + 1];
                     lam[s][2] = r[3 + 3 * s + 2];
                 }
+                // phase 1 (every pair): separation and the r > 2a scalars of Eq. (9)
+                PairCoef<V> c[T];
+                V rxy2[T], r2[T], f[T], G[T];
+                bool near = false;
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    PairCoef<V> c;
-                    pair_coef<L, WALL>(xi[t], yi[t], zi[t], xj, yj, zj, c);
+                    c[t].dx = L::sub(xi[t], xj);
+                    c[t].dy = L::sub(yi[t], yj);
+                    c[t].dz = L::sub(zi[t], zj);
+                    rpy_far_scalars<L>(c[t].dx, c[t].dy, c[t].dz, rxy2[t], r2[t], f[t], G[t]);
+                    near = near || L::any_le(r2[t], 4.0);
+                }
+                // phase 2 (rare, warp-uniform): some lane has an overlapping pair (r <= 2a) or r = 0
+                if (__any_sync(0xffffffffu, near)) {
+#pragma unroll
+                    for (int t = 0; t < T; ++t) rpy_near_fixup<L>(r2[t], f[t], G[t]);
+                }
+                // phase 3 (every pair): wall scalars and the product with lambda_j
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    if constexpr (WALL) wall_coef<L>(zi[t], zj, rxy2[t], f[t], G[t], c[t]);
+                    else { c[t].al = f[t]; c[t].be = G[t]; }
 #pragma unroll
                     for (int s = 0; s < K; ++s)
-                        pair_apply<L, WALL>(c, lam[s][0], lam[s][1], lam[s][2],
+                        pair_apply<L, WALL>(c[t], lam[s][0], lam[s][1], lam[s][2],
                                             acc[t][s][0], acc[t][s][1], acc[t][s][2]);
                 }
             }

@@ -55,6 +55,36 @@ __global__ void __launch_bounds__(kThreads) probe_kernel(int iters, float seed, 
 #pragma unroll
         for (int c = 0; c < kChains; ++c) s += acc[c];
         if (s == 12345.678) sink[0] = s;
+    } else if (KIND == 4) {     // packed FFMA2, three distinct register-pair operands per instruction
+        float2 acc[kChains], x[kChains];
+#pragma unroll
+        for (int c = 0; c < kChains; ++c) {
+            acc[c] = make_float2((float)(threadIdx.x + c), (float)c);
+            x[c] = make_float2(1.0f + seed * (c + 1) * 1e-9f, 1.0f - seed * (c + 2) * 1e-9f);
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) acc[c] = __ffma2_rn(acc[c], x[c], x[(c + 5) % kChains]);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int c = 0; c < kChains; ++c) s += acc[c].x + acc[c].y;
+        if (s == 12345.678f) sink[0] = s;
+    } else if (KIND == 5) {     // scalar FFMA, three distinct register operands per instruction
+        float acc[kChains], x[kChains];
+#pragma unroll
+        for (int c = 0; c < kChains; ++c) {
+            acc[c] = (float)(threadIdx.x + c);
+            x[c] = 1.0f + seed * (c + 1) * 1e-9f;
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) acc[c] = fmaf(acc[c], x[c], x[(c + 5) % kChains]);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int c = 0; c < kChains; ++c) s += acc[c];
+        if (s == 12345.678f) sink[0] = s;
     } else {                    // MUFU.RSQ
         float acc[kChains];
 #pragma unroll
@@ -75,7 +105,7 @@ __global__ void __launch_bounds__(kThreads) probe_kernel(int iters, float seed, 
 extern "C" rpy_status rpy_pipe_peak_probe(int kind, int iters, void* d_sink, float* h_elapsed_ms,
                                           double* h_fma_count, void* cuda_stream)
 {
-    if (kind < 0 || kind > 3 || iters < 1) return RPY_ERR_ARG;
+    if (kind < 0 || kind > 5 || iters < 1) return RPY_ERR_ARG;
     if (!d_sink || !h_elapsed_ms || !h_fma_count) return RPY_ERR_NULL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     cudaEvent_t e0, e1;
@@ -87,6 +117,8 @@ extern "C" rpy_status rpy_pipe_peak_probe(int kind, int iters, void* d_sink, flo
             case 0: probe_kernel<0><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
             case 1: probe_kernel<1><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
             case 2: probe_kernel<2><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
+            case 4: probe_kernel<4><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
+            case 5: probe_kernel<5><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
             default: probe_kernel<3><<<grid, kThreads, 0, st>>>(n, 0.f, sink); break;
         }
     };
@@ -102,7 +134,7 @@ extern "C" rpy_status rpy_pipe_peak_probe(int kind, int iters, void* d_sink, flo
     cudaEventDestroy(e1);
     if (e != cudaSuccess) return RPY_ERR_CUDA;
     *h_elapsed_ms = ms;
-    double per_thread = (double)iters * kChains * (kind == 1 ? 2.0 : 1.0);
+    double per_thread = (double)iters * kChains * ((kind == 1 || kind == 4) ? 2.0 : 1.0);
     *h_fma_count = per_thread * kThreads * (double)grid.x;
     return RPY_OK;
 }
