@@ -42,13 +42,19 @@ if ROOT not in sys.path:
 METRIC = "wall_rpy_matvec_blob_pairs_per_s"
 UNIT = "G blob-pairs/s"
 
-# Algorithmic work of the all-pairs kernel per ordered pair (recounted from
-# the SASS of the built kernels: FMA-pipe lane-instructions and flops with FMA = 2, MUL/ADD = 1).
-# k right-hand sides: geometry part + per-RHS apply part.
+# Work of the all-pairs kernel per ordered pair: FP-pipe lane operations
+# (one per FFMA/FMUL/FADD lane; a packed FFMA2 counts two) and flops (FMA = 2, MUL/ADD = 1) that the
+# kernel EXECUTES on the every-pair path, measured with ncu (per-opcode "Thread Instructions
+# Executed" of the source page / N^2, profiles/*_allpairs_*.md) and equal to the count of the
+# expression tree in csrc/rpy_math.cuh.  k right-hand sides: geometry part + per-RHS apply part.
+# The fp64 path executes the same tree plus five DFMA-pipe operations per reciprocal square root
+# (MUFU.RSQ64H seed + one cubic Newton step): two roots for the wall tensor, one for free space.
 WORK = {
-    # variant: (instr_geom, instr_per_rhs, flop_geom, flop_per_rhs)
-    "wall": (56, 10, 89, 18),
-    "free": (15, 10, 23, 18),
+    # (prec, variant): (lane_ops_geom, lane_ops_per_rhs, flop_geom, flop_per_rhs)
+    ("f32", "wall"): (50, 10, 82, 18),
+    ("f32", "free"): (12, 10, 19, 18),
+    ("f64", "wall"): (59, 10, 95, 18),
+    ("f64", "free"): (17, 10, 24, 18),
 }
 SM_COUNT = 148
 LANES = {"f32": 128, "f64": 64}
@@ -59,8 +65,8 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
-def work_per_pair(variant: str, k: int):
-    ig, ir, fg, fr = WORK[variant]
+def work_per_pair(prec: str, variant: str, k: int):
+    ig, ir, fg, fr = WORK[(prec, variant)]
     return ig + ir * k, fg + fr * k
 
 
@@ -195,26 +201,22 @@ def run_reference(args):
 # ------------------------------------------------------------------------------- GPU leg
 def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, rank=0, world=1, dist=None):
     """Device-resident timing of `steps` calls; returns dict with ms per step (max over ranks)."""
+    from paper_1602_02170_b200 import sharding
     dt = torch.float32 if prec == "f32" else torch.float64
     dev = torch.device("cuda", torch.cuda.current_device())
     pos = torch.from_numpy(wl.pos).to(dt).to(dev)
     force = torch.from_numpy(wl.force).to(dt).to(dev)
     n, k = wl.n_blobs, wl.n_rhs
     fn = binding.rpy_wall_matvec if variant == "wall" else binding.rpy_free_matvec
-    rb = rank * n // world
-    re_ = (rank + 1) * n // world
-    rows = None if world == 1 else (rb, re_ - rb)
+    rows = None if world == 1 else sharding.shard_rows(n, rank, world)
     ws = torch.empty(binding.rpy_matvec_workspace_bytes(prec, n, k), dtype=torch.uint8, device=dev)
     out = torch.empty((k, n if rows is None else rows[1], 3), dtype=dt, device=dev)
-    gathered = None
-    if world > 1:
-        counts = [((r + 1) * n // world - r * n // world) for r in range(world)]
-        gathered = [torch.empty((k, c, 3), dtype=dt, device=dev) for c in counts]
+    gathered = sharding.gather_buffers(n, k, world, dt, dev) if world > 1 else None
 
     def step():
         fn(pos, force, wl.a, wl.eta, out=out, workspace=ws, rows=rows)
         if world > 1:
-            dist.all_gather(gathered, out)
+            sharding.gather_velocities(out, n, buffers=gathered, concatenate=False)
 
     for _ in range(warmup):
         step()
@@ -305,7 +307,7 @@ def run_ours(args):
     clocks = clk.summary()
     ms = res["ms_per_step"]
     value = n * n / (ms * 1e-3) / 1e9
-    instr, flops = work_per_pair(variant, k)
+    instr, flops = work_per_pair(prec, variant, k)
 
     line = None
     if rank == 0:
@@ -329,7 +331,7 @@ def run_ours(args):
             "bound": "alu", "kernel": "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
             "frac": achieved / peak, "traffic": None,
             "peak_source": f"derived: {SM_COUNT} SM x {LANES[prec]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
-            "flop_per_pair": flops, "fma_pipe_instr_per_pair": instr,
+            "flop_per_pair": flops, "lane_ops_per_pair": instr,
             "pipe_frac": pairs_launch * instr / (k_ms * 1e-3) / lane_peak,
             "kernel_ms": k_ms, "prepack_ms": pre_ms, "finalise_ms": fin_ms,
             "kernel_share_of_step": k_ms / (k_ms + pre_ms + fin_ms) if world == 1 else None,
@@ -371,7 +373,7 @@ def run_ours(args):
                 w2 = workloads.make(cfg)
                 r2 = time_config(torch, binding, w2, p, v, st, 3 if cfg != 4 else 1, flush)
                 km, _, _ = time_allpairs_kernel(torch, binding, r2, w2, v, 2 if cfg != 4 else 1, flush)
-                i2, f2 = work_per_pair(v, w2.n_rhs)
+                i2, f2 = work_per_pair(p, v, w2.n_rhs)
                 lane2 = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
                 extra.append({"workload": w2.name, "prec": p, "variant": v, "n_blobs": w2.n_blobs, "n_rhs": w2.n_rhs,
                               "ms_per_step": r2["ms_per_step"], "gps": r2["gps"], "pair_rhs_gps": r2["gps"] * w2.n_rhs,
