@@ -14,7 +14,7 @@ thread_local int g_last_cuda_error = 0;
 
 constexpr int kAbiVersion = 1;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
-constexpr int kTargetCtas = kNumSMs * 16;  // CTAs wanted before sources are no longer chunked
+constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
 constexpr int kMaxChunks = 64;
 constexpr int kBlock = 128;
 constexpr int kMaxT = 2;
@@ -55,25 +55,45 @@ inline size_t record_bytes(rpy_prec prec, int K)
     return (size_t)((raw + per16 - 1) / per16 * per16) * elem_size(prec);
 }
 
+// Two targets per thread once there are enough rows to fill the chip that way (K >= 4 already
+// holds 3K accumulators per target: one target per thread there).
+inline int choose_T(int K, int64_t rows)
+{
+    return (K <= 2 && rows >= (int64_t)kNumSMs * kBlock * 2 * 2) ? 2 : 1;
+}
+
+// The source range is cut into n_chunks so that the CTAs spread evenly over the 148 SMs.  The
+// kernel is ALU-bound and every CTA does the same work, so the time is set by the SM that is
+// handed the most CTAs, m = ceil(CTAs / 148), and by how long the last CTAs run on a partly empty
+// SM.  Measured on B200 (cfg 2, cfg 3, both precisions, 4..64 chunks): throughput rises
+// monotonically with the CTA count up to ~64 CTAs per SM (cfg 3 fp32: 496 G pairs/s at 18 CTAs
+// per SM, 519 at 64+; the fixed cost of a CTA is far below one tile), so: aim for kTargetCtas,
+// and among the chunk counts in the upper half of the allowed range take the one with the least
+// quantisation loss tiles_per_chunk * m.
 Plan make_plan(rpy_prec prec, int64_t n, int K, int64_t rows)
 {
     Plan p;
     p.tile_sources = tile_sources_of(prec);
     p.n_padded = (n + p.tile_sources - 1) / p.tile_sources * p.tile_sources;
     p.n_tiles = p.n_padded / p.tile_sources;
-    // two targets per thread once there are enough rows to fill the chip that way
-    // (K >= 4 already holds 3K accumulators per target: one target per thread there)
-    p.T = (K <= 2 && rows >= (int64_t)kNumSMs * kBlock * 2 * 2) ? 2 : 1;
+    p.T = choose_T(K, rows);
     p.targets_per_cta = kBlock * p.T;
     p.n_target_tiles = (rows + p.targets_per_cta - 1) / p.targets_per_cta;
-    int64_t want = p.n_target_tiles > 0 ? (kTargetCtas + p.n_target_tiles - 1) / p.n_target_tiles : 1;
-    if (want > kMaxChunks) want = kMaxChunks;
-    if (want > p.n_tiles) want = p.n_tiles;
-    if (want < 1) want = 1;
-    p.tiles_per_chunk = (int)((p.n_tiles + want - 1) / want);
-    if (p.tiles_per_chunk < 1) p.tiles_per_chunk = 1;
-    p.n_chunks = (int)((p.n_tiles + p.tiles_per_chunk - 1) / p.tiles_per_chunk);
-    if (p.n_chunks < 1) p.n_chunks = 1;
+    int64_t c_max = p.n_target_tiles > 0 ? (kTargetCtas + p.n_target_tiles - 1) / p.n_target_tiles : 1;
+    if (c_max > kMaxChunks) c_max = kMaxChunks;
+    if (c_max > p.n_tiles) c_max = p.n_tiles;
+    if (c_max < 1) c_max = 1;
+    int64_t best_cost = -1;
+    p.tiles_per_chunk = (int)p.n_tiles; p.n_chunks = 1;
+    for (int64_t want = (c_max + 1) / 2; want <= c_max; ++want) {
+        int64_t tpc = (p.n_tiles + want - 1) / want;
+        int64_t nch = (p.n_tiles + tpc - 1) / tpc;
+        int64_t per_sm = (p.n_target_tiles * nch + kNumSMs - 1) / kNumSMs;
+        int64_t cost = tpc * per_sm;
+        if (best_cost < 0 || cost <= best_cost) {
+            best_cost = cost; p.tiles_per_chunk = (int)tpc; p.n_chunks = (int)nch;
+        }
+    }
     return p;
 }
 
@@ -88,16 +108,21 @@ size_t records_bytes(rpy_prec prec, int64_t n, int K)
 }
 
 // n_chunks * rows <= kTargetCtas * kBlock * kMaxT + rows  (n_chunks <= kTargetCtas / n_target_tiles + 1)
-size_t partial_bytes_bound(int64_t n, int K)
+// and n_chunks <= n_tiles, rows <= n.
+size_t partial_bytes_bound(rpy_prec prec, int64_t n, int K)
 {
-    return align_up((size_t)((int64_t)kTargetCtas * kBlock * kMaxT + n) * (size_t)K * 3 * sizeof(double), kAlign);
+    int ts = tile_sources_of(prec);
+    int64_t n_tiles = (n + ts - 1) / ts;
+    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + n;
+    int64_t b = n_tiles * n;
+    return align_up((size_t)(a < b ? a : b) * (size_t)K * 3 * sizeof(double), kAlign);
 }
 
 size_t workspace_bytes(rpy_prec prec, int64_t n, int n_rhs)
 {
     if (n <= 0 || n_rhs < 1) return 0;
     int K = group_k(n_rhs);
-    return records_bytes(prec, n, K) + partial_bytes_bound(n, K);
+    return records_bytes(prec, n, K) + partial_bytes_bound(prec, n, K);
 }
 
 inline rpy_status cuda_fail(cudaError_t e)
@@ -113,20 +138,24 @@ inline bool overlaps(const void* p, size_t pn, const void* q, size_t qn)
 }
 
 template <class L, int K, bool WALL, int T>
+auto allpairs_fn()
+{
+    using Sh = Shape<L, K>;
+    return rpy::allpairs_kernel<L, K, WALL, T, kBlock, Sh::TILE_G, Sh::FLUSH_G, Sh::MINB>;
+}
+template <class L, int K> constexpr size_t allpairs_smem() { return 2 * (size_t)Shape<L, K>::TILE_G * rpy::RecLayout<L, K>::BYTES; }
+
+template <class L, int K, bool WALL, int T>
 cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, double* partial,
                             int64_t row_begin, int64_t rows, cudaStream_t st)
 {
-    using Sh = Shape<L, K>;
-    constexpr int TILE_G = Sh::TILE_G;
-    auto kern = rpy::allpairs_kernel<L, K, WALL, T, kBlock, TILE_G, Sh::FLUSH_G, Sh::MINB>;
-    size_t smem = 2 * (size_t)TILE_G * rpy::RecLayout<L, K>::BYTES;
     dim3 grid((unsigned)p.n_target_tiles, (unsigned)p.n_chunks);
-    kern<<<grid, kBlock, smem, st>>>(rec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
+    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
     return cudaGetLastError();
 }
 
 template <class L, int K>
-cudaError_t run_group(bool wall, const Plan& p, int64_t n, int64_t row_begin, int64_t rows,
+cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, typename L::S* vel,
                       double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev)
 {
@@ -134,6 +163,7 @@ cudaError_t run_group(bool wall, const Plan& p, int64_t n, int64_t row_begin, in
     S* rec = reinterpret_cast<S*>(ws);
     rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
     double* partial = reinterpret_cast<double*>(ws + records_bytes(prec, n, K));
+    const Plan p = make_plan(prec, n, K, rows);
     {
         int threads = 256;
         int64_t blocks = (p.n_padded + threads - 1) / threads;
@@ -144,7 +174,7 @@ cudaError_t run_group(bool wall, const Plan& p, int64_t n, int64_t row_begin, in
     }
     cudaError_t e;
     if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
-    constexpr int T2 = K <= 2 ? 2 : 1;     // make_plan never asks for T = 2 when K > 2
+    constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
     if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, partial, row_begin, rows, st)
                            : launch_allpairs<L, K, true, 1>(p, rec, partial, row_begin, rows, st);
     else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, partial, row_begin, rows, st)
@@ -170,7 +200,6 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
                            double a, double eta, void* ws, cudaStream_t st, void* const* ev)
 {
     using S = typename L::S;
-    rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
     cudaError_t ee;
     if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[0]), st)) != cudaSuccess) return ee;
     const S* pos = static_cast<const S*>(d_pos);
@@ -180,13 +209,12 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
         const S* force = static_cast<const S*>(d_force) + (int64_t)done * n * 3;
         S* vel = static_cast<S*>(d_vel) + (int64_t)done * rows * 3;
         unsigned char* w = static_cast<unsigned char*>(ws);
-        Plan p = make_plan(prec, n, K, rows);
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            case 4: e = run_group<L, 4>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            case 2: e = run_group<L, 2>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            default: e = run_group<L, 1>(wall, p, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
