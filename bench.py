@@ -65,8 +65,12 @@ def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
-def work_per_pair(prec: str, variant: str, k: int):
+def work_per_pair(prec: str, variant: str, k: int, symmetric: bool = False):
+    """(FP-pipe lane operations, flops) per ORDERED pair.  The symmetric kernel builds the geometry
+    and the coefficients once per unordered pair and applies them twice (M_ij and M_ij^T)."""
     ig, ir, fg, fr = WORK[(prec, variant)]
+    if symmetric:
+        return (ig + 2 * ir * k) / 2, (fg + 2 * fr * k) / 2
     return ig + ir * k, fg + fr * k
 
 
@@ -307,7 +311,8 @@ def run_ours(args):
     clocks = clk.summary()
     ms = res["ms_per_step"]
     value = n * n / (ms * 1e-3) / 1e9
-    instr, flops = work_per_pair(prec, variant, k)
+    plan = binding.rpy_matvec_launch_plan(prec, n, k, n // world if world > 1 else n)
+    instr, flops = work_per_pair(prec, variant, k, plan["symmetric"])
 
     line = None
     if rank == 0:
@@ -328,7 +333,7 @@ def run_ours(args):
             probe = {"error": str(e)}
         lane_peak = SM_COUNT * LANES[prec] * SM_MAX_GHZ * 1e9
         roofline = {
-            "bound": "alu", "kernel": "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "bound": "alu", "kernel": "allpairs_sym_kernel" if plan["symmetric"] else "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
             "frac": achieved / peak, "traffic": None,
             "peak_source": f"derived: {SM_COUNT} SM x {LANES[prec]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
             "flop_per_pair": flops, "lane_ops_per_pair": instr,
@@ -346,7 +351,6 @@ def run_ours(args):
         if world == 1 and not args.no_cpu:
             gps, cores, desc, t, _ = oracle_sample(wl, variant, prec, 15.0)
             cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
-        plan = binding.rpy_matvec_launch_plan(prec, n, k, n // world if world > 1 else n)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
@@ -373,11 +377,12 @@ def run_ours(args):
                 w2 = workloads.make(cfg)
                 r2 = time_config(torch, binding, w2, p, v, st, 3 if cfg != 4 else 1, flush)
                 km, _, _ = time_allpairs_kernel(torch, binding, r2, w2, v, 2 if cfg != 4 else 1, flush)
-                i2, f2 = work_per_pair(p, v, w2.n_rhs)
+                pl2 = binding.rpy_matvec_launch_plan(p, w2.n_blobs, w2.n_rhs, w2.n_blobs)
+                i2, f2 = work_per_pair(p, v, w2.n_rhs, pl2["symmetric"])
                 lane2 = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
                 extra.append({"workload": w2.name, "prec": p, "variant": v, "n_blobs": w2.n_blobs, "n_rhs": w2.n_rhs,
                               "ms_per_step": r2["ms_per_step"], "gps": r2["gps"], "pair_rhs_gps": r2["gps"] * w2.n_rhs,
-                              "kernel_ms": km,
+                              "kernel_ms": km, "symmetric": pl2["symmetric"],
                               "pipe_frac": w2.n_blobs ** 2 * i2 / (km * 1e-3) / lane2,
                               "flop_frac": w2.n_blobs ** 2 * f2 / (km * 1e-3) / 1e12 / peak_tflops(p)})
                 log(f"[bench] extra {extra[-1]}")

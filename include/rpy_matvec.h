@@ -152,12 +152,21 @@ rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs
                              void *d_workspace, size_t workspace_bytes, void *cuda_stream,
                              void *const *cuda_events4);
 
-/* Launch geometry the all-pairs kernel would use for (prec, n_blobs, n_rhs, row_count):
- * targets per CTA, number of source chunks, sources per shared-memory tile, CTAs.
- * Pure host arithmetic (no CUDA call); any output pointer may be NULL. */
+/* Launch geometry the all-pairs kernel would use for (prec, n_blobs, n_rhs, row_count).
+ * Pure host arithmetic (no CUDA call); any output pointer may be NULL.
+ *   *symmetric == 0: the plain kernel.  A CTA owns *targets_per_cta target rows and walks one of
+ *     *n_source_chunks contiguous chunks of the sources in shared-memory tiles of *tile_sources.
+ *   *symmetric == 1: the symmetric kernel (n_rhs == 1, all rows, n_blobs >= 6,144), which uses
+ *     M_ij = M_ji^T to build every unordered pair's coefficients once.  Blobs are
+ *     cut into tiles of *tile_sources (= *targets_per_cta); a CTA owns one tile I and walks the
+ *     tiles (I + d) mod n_tiles for one of *n_source_chunks chunks of the distances d = 0..n_tiles/2.
+ *     The transposed half of the sum is accumulated with fp64 atomics, so the result is
+ *     reproducible to rounding of the double sums (~1e-16 relative), not bit for bit; the plain
+ *     kernel (and therefore every *_rows call and every n_rhs > 1 call) is bit-reproducible.
+ *   *n_ctas: CTAs of the launch. */
 rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_count,
                                   int *targets_per_cta, int *n_source_chunks,
-                                  int *tile_sources, int64_t *n_ctas);
+                                  int *tile_sources, int64_t *n_ctas, int *symmetric);
 
 const char *rpy_status_string(rpy_status s);
 

@@ -53,7 +53,7 @@ SIGNATURES = {
     "rpy_pipe_peak_probe": (_int, [_int, _int, _vp, ctypes.POINTER(ctypes.c_float),
                                    ctypes.POINTER(ctypes.c_double), _vp]),
     "rpy_matvec_launch_plan": (_int, [_int, _i64, _int, _i64, ctypes.POINTER(_int), ctypes.POINTER(_int),
-                                      ctypes.POINTER(_int), ctypes.POINTER(_i64)]),
+                                      ctypes.POINTER(_int), ctypes.POINTER(_i64), ctypes.POINTER(_int)]),
     "rpy_matvec_phases": (_int, [_int, _int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp,
                                  ctypes.POINTER(_vp)]),
     "rpy_status_string": (ctypes.c_char_p, [_int]),
@@ -121,12 +121,13 @@ def rpy_matvec_host_scratch_bytes(prec, n_blobs: int, n_rhs: int = 1) -> int:
 def rpy_matvec_launch_plan(prec, n_blobs: int, n_rhs: int = 1, row_count: Optional[int] = None) -> dict:
     """Launch geometry of the all-pairs kernel (pure host arithmetic, works without a GPU)."""
     lib = load_library()
-    tpc, nch, ts, nct = _int(), _int(), _int(), _i64()
+    tpc, nch, ts, nct, sym = _int(), _int(), _int(), _i64(), _int()
     rc = n_blobs if row_count is None else row_count
     _check(lib.rpy_matvec_launch_plan(_prec_code(prec), int(n_blobs), int(n_rhs), int(rc),
-                                      ctypes.byref(tpc), ctypes.byref(nch), ctypes.byref(ts), ctypes.byref(nct)))
+                                      ctypes.byref(tpc), ctypes.byref(nch), ctypes.byref(ts), ctypes.byref(nct),
+                                      ctypes.byref(sym)))
     return {"targets_per_cta": tpc.value, "n_source_chunks": nch.value, "tile_sources": ts.value,
-            "n_ctas": nct.value}
+            "n_ctas": nct.value, "symmetric": bool(sym.value)}
 
 
 def _require_cuda(t: torch.Tensor, what: str):

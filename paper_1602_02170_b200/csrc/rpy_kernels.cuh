@@ -243,6 +243,199 @@ allpairs_kernel(const typename L::S* __restrict__ rec, double* __restrict__ part
     }
 }
 
+// ---------------------------------------------------------------------------- all-pairs, symmetric
+// Uses M_ij = M_ji^T (M is symmetric by construction of Eq. (7)): the five pair
+// coefficients of the unordered pair {i, j} are built ONCE and applied twice,
+//   u_i += M_ij lambda_j   (forward,    accumulators stay with the thread that owns target i),
+//   u_j += M_ij^T lambda_i (transposed, accumulators TRAVEL with the source),
+// which costs 50 + 2*10 FP-pipe operations per unordered pair instead of 2*(50 + 10).
+//
+// Decomposition.  Blobs are cut into tiles of TS = BLOCK*T; tile I meets tile J = (I + d) mod nt
+// for d = 0 .. nt/2: every unordered tile pair exactly once (for even nt the distance nt/2 is
+// taken by I < nt/2 only), every I the same amount of work.  Grid: x = I, y = chunk of the d range.
+// d = 0 is the diagonal tile: all TS x TS ordered pairs are walked forward with the transposed
+// application switched off (lambda_i := 0 there).
+//
+// Inside a tile pair each thread owns T targets of I.  A warp walks J in sub-tiles of 32 source
+// groups: at step s lane l reads group (s + l) mod 32 from shared memory (each lane a different
+// 48-byte record: bank-conflict-free) and holds that group's transposed
+// accumulators, which it hands to lane l-1 by one warp shuffle per component after the step.
+// After 32 steps every group has met all 32*T targets of the warp and is back in its home lane,
+// which adds the float partial (<= 32*T terms) into the double array `gacc` with one fp64 atomic
+// per component: the order of those atomics is the only non-deterministic part of the result.
+// The four warps start on different sub-tiles so they never flush the same addresses together.
+template <class V> __device__ __forceinline__ V shfl_from(V v, int src_lane);
+template <> __device__ __forceinline__ double shfl_from<double>(double v, int src_lane) { return __shfl_sync(0xffffffffu, v, src_lane); }
+template <> __device__ __forceinline__ float shfl_from<float>(float v, int src_lane) { return __shfl_sync(0xffffffffu, v, src_lane); }
+template <> __device__ __forceinline__ float2 shfl_from<float2>(float2 v, int src_lane)
+{
+    return make_float2(__shfl_sync(0xffffffffu, v.x, src_lane), __shfl_sync(0xffffffffu, v.y, src_lane));
+}
+template <class V> __device__ __forceinline__ double lane_elem(V v, int w);
+template <> __device__ __forceinline__ double lane_elem<double>(double v, int) { return v; }
+template <> __device__ __forceinline__ double lane_elem<float>(float v, int) { return (double)v; }
+template <> __device__ __forceinline__ double lane_elem<float2>(float2 v, int w) { return (double)(w ? v.y : v.x); }
+
+template <class L, bool WALL, int T, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial, double* __restrict__ gacc,
+                    int64_t n_blobs, int nt, int d_per_chunk)
+{
+    using V = typename L::V;
+    using S = typename L::S;
+    using R = RecLayout<L, 1>;
+    constexpr int W = L::W;
+    constexpr bool IS_F64 = sizeof(S) == 8;
+    constexpr int TS = BLOCK * T;                  // blobs per tile
+    constexpr int TILE_G = TS / W;                 // records per tile
+    constexpr int NSUB = TILE_G / 32;              // sub-tiles of 32 records
+    constexpr int NWARP = BLOCK / 32;
+    constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
+    static_assert(TILE_G % 32 == 0 && R::LEN * sizeof(S) == 48, "record geometry");
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* const buf0 = smem_raw;
+    __shared__ __align__(8) uint64_t full_bar[2];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int I = blockIdx.x;
+    const int D = nt / 2;                          // largest tile distance
+    const int d_lo = blockIdx.y * d_per_chunk;
+    int d_hi = d_lo + d_per_chunk;
+    if (d_hi > D + 1) d_hi = D + 1;
+    if ((nt & 1) == 0 && d_hi == D + 1 && I >= D && D > 0) d_hi = D;   // distance nt/2: lower half only
+    if (nt == 1) d_hi = d_lo == 0 ? 1 : 0;
+    const int my_tiles = d_hi - d_lo;
+
+    if (tid == 0) {
+        mbar_init(&full_bar[0], 1);
+        mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const unsigned char* gbase = reinterpret_cast<const unsigned char*>(rec);
+    auto tile_of = [&](int it) { int J = I + d_lo + it; return J >= nt ? J - nt : J; };
+    if (tid == 0 && my_tiles > 0) {
+        mbar_expect_tx(&full_bar[0], TILE_BYTES);
+        bulk_g2s(buf0, gbase + (int64_t)tile_of(0) * TILE_BYTES, TILE_BYTES, &full_bar[0]);
+    }
+
+    V xi[T], yi[T], zi[T], li[T][3];
+    int64_t row[T];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        row[t] = (int64_t)I * TS + t * BLOCK + tid;            // < n_padded: a real record (maybe padding)
+        const S* r = rec + (row[t] / W) * R::LEN + (row[t] % W);
+        xi[t] = L::bc((double)r[0 * W]);
+        yi[t] = L::bc((double)r[1 * W]);
+        zi[t] = L::bc((double)r[2 * W]);
+        li[t][0] = L::bc((double)r[3 * W]);
+        li[t][1] = L::bc((double)r[4 * W]);
+        li[t][2] = L::bc((double)r[5 * W]);
+    }
+
+    double dacc[IS_F64 ? 1 : T][3];
+    V acc[T][3];
+#pragma unroll
+    for (int t = 0; t < T; ++t)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            acc[t][c] = L::bc(0.0);
+            if constexpr (!IS_F64) dacc[t][c] = 0.0;
+        }
+
+    for (int it = 0; it < my_tiles; ++it) {
+        const int b = it & 1;
+        __syncthreads();                                       // buffer b^1 is free again
+        if (tid == 0 && it + 1 < my_tiles) {
+            mbar_expect_tx(&full_bar[b ^ 1], TILE_BYTES);
+            bulk_g2s(buf0 + (b ^ 1) * TILE_BYTES, gbase + (int64_t)tile_of(it + 1) * TILE_BYTES, TILE_BYTES, &full_bar[b ^ 1]);
+        }
+        mbar_wait(&full_bar[b], (uint32_t)((it >> 1) & 1));
+        const S* tile = reinterpret_cast<const S*>(buf0 + b * TILE_BYTES);
+        const int J = tile_of(it);
+        const bool diagonal = (d_lo + it) == 0;
+        V lt[T][3];                                            // lambda_i as seen by the transposed application
+#pragma unroll
+        for (int t = 0; t < T; ++t)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) lt[t][c] = diagonal ? L::bc(0.0) : li[t][c];
+
+#pragma unroll 1
+        for (int p = 0; p < NSUB; ++p) {
+            const int q = (p + warp * (NSUB / NWARP > 0 ? NSUB / NWARP : 1)) % NSUB;
+            const S* sub = tile + (q * 32) * R::LEN;
+            V uj[3] = {L::bc(0.0), L::bc(0.0), L::bc(0.0)};
+#pragma unroll 2
+            for (int s = 0; s < 32; ++s) {
+                const int g = (s + lane) & 31;
+                const V* r = reinterpret_cast<const V*>(sub + g * R::LEN);
+                V xj = r[0], yj = r[1], zj = r[2];
+                V lj0 = r[3], lj1 = r[4], lj2 = r[5];
+                PairCoef<V> c[T];
+                V rxy2[T], r2[T], f[T], G[T];
+                bool near = false;
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    c[t].dx = L::sub(xi[t], xj);
+                    c[t].dy = L::sub(yi[t], yj);
+                    c[t].dz = L::sub(zi[t], zj);
+                    rpy_far_scalars<L>(c[t].dx, c[t].dy, c[t].dz, rxy2[t], r2[t], f[t], G[t]);
+                    near = near || L::any_le(r2[t], 4.0);
+                }
+                if (__any_sync(0xffffffffu, near)) {
+#pragma unroll
+                    for (int t = 0; t < T; ++t) rpy_near_fixup<L>(r2[t], f[t], G[t]);
+                }
+#pragma unroll
+                for (int t = 0; t < T; ++t) {
+                    if constexpr (WALL) wall_coef<L>(zi[t], zj, rxy2[t], f[t], G[t], c[t]);
+                    else { c[t].al = f[t]; c[t].be = G[t]; }
+                    pair_apply<L, WALL>(c[t], lj0, lj1, lj2, acc[t][0], acc[t][1], acc[t][2]);
+                    if constexpr (WALL) { V tmp = c[t].ga; c[t].ga = c[t].ep; c[t].ep = tmp; }   // M^T: xz <-> zx
+                    pair_apply<L, WALL>(c[t], lt[t][0], lt[t][1], lt[t][2], uj[0], uj[1], uj[2]);
+                }
+                const int from = (lane + 1) & 31;              // the lane that just served group g + 1
+                uj[0] = shfl_from<V>(uj[0], from);
+                uj[1] = shfl_from<V>(uj[1], from);
+                uj[2] = shfl_from<V>(uj[2], from);
+            }
+            // home again: lane holds the sum over this warp's 32*T targets for record q*32 + lane
+            if (!diagonal) {
+#pragma unroll
+                for (int w = 0; w < W; ++w) {
+                    int64_t j = (int64_t)J * TS + (int64_t)(q * 32 + lane) * W + w;
+                    if (j < n_blobs) {
+                        atomicAdd(gacc + j * 3 + 0, lane_elem<V>(uj[0], w));
+                        atomicAdd(gacc + j * 3 + 1, lane_elem<V>(uj[1], w));
+                        atomicAdd(gacc + j * 3 + 2, lane_elem<V>(uj[2], w));
+                    }
+                }
+            }
+            if constexpr (!IS_F64) {
+#pragma unroll
+                for (int t = 0; t < T; ++t)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        dacc[t][c] += L::hsum(acc[t][c]);
+                        acc[t][c] = L::bc(0.0);
+                    }
+            }
+        }
+    }
+
+    double* out = partial + (int64_t)blockIdx.y * n_blobs * 3;
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        if (row[t] < n_blobs) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                if constexpr (IS_F64) out[row[t] * 3 + c] = L::hsum(acc[t][c]);
+                else                  out[row[t] * 3 + c] = dacc[t][c];
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------- finalise
 // vel[s][row][c] = scale * sum_{chunk} partial[chunk][s][row][c], chunks added in index order
 // (deterministic), one thread per output element.

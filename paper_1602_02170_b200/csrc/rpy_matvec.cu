@@ -8,17 +8,26 @@
 #include "../../include/rpy_matvec.h"
 #include "rpy_kernels.cuh"
 
+#ifndef RPY_SYM_MINB_F32
+#define RPY_SYM_MINB_F32 3
+#endif
+#ifndef RPY_SYM_MINB_F64
+#define RPY_SYM_MINB_F64 3
+#endif
+
 namespace {
 
 thread_local int g_last_cuda_error = 0;
 
-constexpr int kAbiVersion = 1;
+constexpr int kAbiVersion = 2;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
 constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
 constexpr int kMaxChunks = 64;
 constexpr int kBlock = 128;
 constexpr int kMaxT = 2;
 constexpr size_t kAlign = 256;
+constexpr int kSymTile = kBlock * 2;       // blobs per tile of the symmetric kernel (T = 2)
+constexpr int64_t kSymMinBlobs = 24 * kSymTile;   // below this the plain kernel is used (too few tile pairs per CTA)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -101,7 +110,7 @@ inline int group_k(int remaining) { return remaining >= 8 ? 8 : remaining >= 4 ?
 
 size_t records_bytes(rpy_prec prec, int64_t n, int K)
 {
-    int ts = tile_sources_of(prec);
+    int ts = kSymTile;                       // a multiple of every kernel's tile (64 / 128 / 256 sources)
     int64_t n_padded = (n + ts - 1) / ts * ts;
     int W = prec == RPY_PREC_F64 ? 1 : 2;
     return align_up((size_t)(n_padded / W) * record_bytes(prec, K), kAlign);
@@ -113,7 +122,7 @@ size_t partial_bytes_bound(rpy_prec prec, int64_t n, int K)
 {
     int ts = tile_sources_of(prec);
     int64_t n_tiles = (n + ts - 1) / ts;
-    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + n;
+    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + 2 * n;   // symmetric path: chunks + 1 slices
     int64_t b = n_tiles * n;
     return align_up((size_t)(a < b ? a : b) * (size_t)K * 3 * sizeof(double), kAlign);
 }
@@ -154,6 +163,44 @@ cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, double* par
     return cudaGetLastError();
 }
 
+// Symmetric path (rpy::allpairs_sym_kernel): one right-hand side, all rows, enough tiles.
+struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; };
+
+inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
+{
+    return K == 1 && row_begin == 0 && rows == n && n >= kSymMinBlobs;
+}
+
+SymPlan make_sym_plan(int64_t n)
+{
+    SymPlan p;
+    p.n_padded = (n + kSymTile - 1) / kSymTile * kSymTile;
+    p.nt = (int)(p.n_padded / kSymTile);
+    int count = p.nt / 2 + 1;                                  // tile distances 0 .. nt/2
+    int64_t want = (kTargetCtas + p.nt - 1) / p.nt;
+    if (want > count) want = count;
+    if (want < 1) want = 1;
+    p.d_per_chunk = (int)((count + want - 1) / want);
+    p.n_chunks = (count + p.d_per_chunk - 1) / p.d_per_chunk;
+    return p;
+}
+
+template <class L> struct SymShape;
+template <> struct SymShape<rpy::Lane<float2>> { static constexpr int MINB = RPY_SYM_MINB_F32; };
+template <> struct SymShape<rpy::Lane<double>> { static constexpr int MINB = RPY_SYM_MINB_F64; };
+
+template <class L>
+cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, double* partial, double* gacc,
+                       int64_t n, cudaStream_t st)
+{
+    constexpr int MINB = SymShape<L>::MINB;
+    size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
+    dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
+    if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk);
+    else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk);
+    return cudaGetLastError();
+}
+
 template <class L, int K>
 cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, typename L::S* vel,
@@ -163,22 +210,36 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     S* rec = reinterpret_cast<S*>(ws);
     rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
     double* partial = reinterpret_cast<double*>(ws + records_bytes(prec, n, K));
+    const bool sym = use_symmetric(n, K, row_begin, rows);
     const Plan p = make_plan(prec, n, K, rows);
+    const SymPlan sp = make_sym_plan(n);
+    const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
     {
         int threads = 256;
-        int64_t blocks = (p.n_padded + threads - 1) / threads;
-        rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, p.n_padded,
+        int64_t blocks = (n_padded + threads - 1) / threads;
+        rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, n_padded,
                                                                       n * 3, 1.0 / a);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     cudaError_t e;
-    if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
-    constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
-    if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, partial, row_begin, rows, st)
-                           : launch_allpairs<L, K, true, 1>(p, rec, partial, row_begin, rows, st);
-    else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, partial, row_begin, rows, st)
-                           : launch_allpairs<L, K, false, 1>(p, rec, partial, row_begin, rows, st);
+    int n_slices = p.n_chunks;
+    if (sym) {
+        // slice n_chunks of `partial` receives the transposed half through fp64 atomics
+        double* gacc = partial + (int64_t)sp.n_chunks * n * 3;
+        if ((e = cudaMemsetAsync(gacc, 0, (size_t)n * 3 * sizeof(double), st)) != cudaSuccess) return e;
+        if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
+        if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, partial, gacc, n, st);
+        else e = cudaErrorInvalidValue;
+        n_slices = sp.n_chunks + 1;
+    } else {
+        if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
+        constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
+        if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, partial, row_begin, rows, st)
+                               : launch_allpairs<L, K, true, 1>(p, rec, partial, row_begin, rows, st);
+        else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, partial, row_begin, rows, st)
+                               : launch_allpairs<L, K, false, 1>(p, rec, partial, row_begin, rows, st);
+    }
     if (e != cudaSuccess) return e;
     if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[2]), st)) != cudaSuccess) return e;
     {
@@ -186,7 +247,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int threads = 256;
         int64_t blocks = (per_chunk + threads - 1) / threads;
         const double PI = 3.14159265358979323846;
-        rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, vel, per_chunk, p.n_chunks,
+        rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, vel, per_chunk, n_slices,
                                                                     rows * 3, rows * 3,
                                                                     1.0 / (6.0 * PI * eta * a));
         e = cudaGetLastError();
@@ -391,15 +452,27 @@ rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void* d_po
 }
 
 rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_count,
-                                  int* targets_per_cta, int* n_source_chunks, int* tile_sources, int64_t* n_ctas)
+                                  int* targets_per_cta, int* n_source_chunks, int* tile_sources, int64_t* n_ctas,
+                                  int* symmetric)
 {
     if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
     if (n_blobs < 0 || n_blobs > RPY_MAX_BLOBS || n_rhs < 1 || row_count < 0 || row_count > n_blobs) return RPY_ERR_ARG;
-    Plan p = make_plan(prec, n_blobs, group_k(n_rhs), row_count);
+    const int K = group_k(n_rhs);
+    if (use_symmetric(n_blobs, K, 0, row_count) && n_rhs == 1) {
+        SymPlan sp = make_sym_plan(n_blobs);
+        if (targets_per_cta) *targets_per_cta = kSymTile;
+        if (n_source_chunks) *n_source_chunks = sp.n_chunks;
+        if (tile_sources) *tile_sources = kSymTile;
+        if (n_ctas) *n_ctas = (int64_t)sp.nt * sp.n_chunks;
+        if (symmetric) *symmetric = 1;
+        return RPY_OK;
+    }
+    Plan p = make_plan(prec, n_blobs, K, row_count);
     if (targets_per_cta) *targets_per_cta = p.targets_per_cta;
     if (n_source_chunks) *n_source_chunks = p.n_chunks;
     if (tile_sources) *tile_sources = p.tile_sources;
     if (n_ctas) *n_ctas = p.n_target_tiles * p.n_chunks;
+    if (symmetric) *symmetric = 0;
     return RPY_OK;
 }
 

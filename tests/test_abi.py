@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), f"{n} declared in the header but not exported"
     assert set(names) == set(binding.SIGNATURES), "binding and header disagree on the symbol list"
-    assert lib.rpy_abi_version() == 1
+    assert lib.rpy_abi_version() == 2
 
 
 def test_no_torch_or_oracle_in_native_symbols():
@@ -71,23 +71,37 @@ def test_launch_plan_covers_all_sources_and_fits_workspace(prec, n, k):
     for rows in sorted({n, max(1, n // 2), 1}):
         p = binding.rpy_matvec_launch_plan(prec, n, k, rows)
         ts, tpc, nch = p["tile_sources"], p["targets_per_cta"], p["n_source_chunks"]
-        n_tiles = -(-n // ts)
-        assert 1 <= nch <= max(1, n_tiles)
-        tiles_per_chunk = -(-n_tiles // nch)
-        assert tiles_per_chunk * nch >= n_tiles                 # every tile is in some chunk
-        assert tiles_per_chunk * (nch - 1) < n_tiles            # no empty chunk
-        assert p["n_ctas"] == -(-rows // tpc) * nch
-        # partial sums [chunk][k][rows][3] doubles + packed records fit the advertised workspace
         kg = 8 if k >= 8 else 4 if k >= 4 else 2 if k >= 2 else 1
         w = 2 if prec == F32 else 1
         es = 4 if prec == F32 else 8
         rec = -(-((3 + 3 * kg) * w * es) // 16) * 16
-        need = (-(-n // ts) * ts // w) * rec + nch * kg * rows * 3 * 8
+        if p["symmetric"]:
+            # symmetric kernel: one RHS, all rows, tiles of 256 blobs, chunks of the tile distances 0..nt/2
+            assert k == 1 and rows == n and n >= 24 * 256 and ts == tpc == 256
+            nt = -(-n // ts)
+            count = nt // 2 + 1
+            assert 1 <= nch <= count
+            d_per_chunk = -(-count // nch)
+            assert d_per_chunk * nch >= count and d_per_chunk * (nch - 1) < count
+            assert p["n_ctas"] == nt * nch
+            # records padded to whole tiles + (chunks + 1) slices of double partials (the extra
+            # slice takes the transposed half)
+            need = (nt * ts // w) * rec + (nch + 1) * n * 3 * 8
+        else:
+            n_tiles = -(-n // ts)
+            assert 1 <= nch <= max(1, n_tiles)
+            tiles_per_chunk = -(-n_tiles // nch)
+            assert tiles_per_chunk * nch >= n_tiles                 # every tile is in some chunk
+            assert tiles_per_chunk * (nch - 1) < n_tiles            # no empty chunk
+            assert p["n_ctas"] == -(-rows // tpc) * nch
+            # partial sums [chunk][k][rows][3] doubles + packed records fit the advertised workspace
+            need = (-(-n // ts) * ts // w) * rec + nch * kg * rows * 3 * 8
         assert need <= binding.rpy_matvec_workspace_bytes(prec, n, k)
     if n >= 172032 and k == 1:
-        assert p is not None
         full = binding.rpy_matvec_launch_plan(prec, n, k, n)
+        assert full["symmetric"]
         assert full["n_ctas"] >= 148 * 4      # enough CTAs for several waves on 148 SMs
+        assert not binding.rpy_matvec_launch_plan(prec, n, k, n - 1)["symmetric"]   # row ranges: plain kernel
 
 
 def test_argument_errors_are_returned_before_any_cuda_work():
@@ -126,7 +140,7 @@ def test_argument_errors_are_returned_before_any_cuda_work():
     assert lib.rpy_wall_count_below(F64, 4, p, 1.0, None, None) == 1
     assert lib.rpy_pipe_peak_probe(9, 10, p, None, None, None) == 2
     assert lib.rpy_pipe_peak_probe(0, 10, None, None, None, None) == 1
-    assert lib.rpy_matvec_launch_plan(F64, 10, 1, 11, None, None, None, None) == 2
+    assert lib.rpy_matvec_launch_plan(F64, 10, 1, 11, None, None, None, None, None) == 2
     assert lib.rpy_last_cuda_error() == 0
 
 

@@ -114,6 +114,41 @@ def test_small_shell_lattice_all_rows(prec):
         check(u, ref, "f32", f"cfg5-small {variant}")
 
 
+# ------------------------------------------------------------------ symmetric kernel (n >= 6,144, k = 1, all rows)
+@pytest.mark.parametrize("variant", ["wall", "free"])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [6144, 6145, 6400 + 77, 7 * 1024 + 1])
+def test_symmetric_kernel_tile_edges(prec, variant, n):
+    """The path that uses M_ij = M_ji^T: even tile count (24: the half-distance case), odd (25),
+    ragged last tile, 29 tiles; dense enough that overlapping pairs (r < 2a) occur across tiles."""
+    assert binding.rpy_matvec_launch_plan(prec, n, 1, n)["symmetric"]
+    rng = np.random.default_rng(300 + n)
+    side = 40.0
+    pos = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(1.1, 9, n)])
+    lam = rng.standard_normal((1, n, 3))
+    u, ref = run_case(pos, lam, prec, variant, a=0.9, eta=1.7)
+    check(u, ref, prec, f"symmetric n={n} {variant}")
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_symmetric_and_plain_kernels_agree(prec):
+    """Same inputs through the symmetric kernel (all rows) and the plain kernel (two row ranges)."""
+    w = workloads.config2(n_bodies=600)          # 9,000 blobs
+    n = w.n_blobs
+    pos = torch.from_numpy(w.pos.astype(NP[prec])).cuda(); lam = torch.from_numpy(w.force.astype(NP[prec])).cuda()
+    assert binding.rpy_matvec_launch_plan(prec, n, 1, n)["symmetric"]
+    assert not binding.rpy_matvec_launch_plan(prec, n, 1, n // 2)["symmetric"]
+    for fn in (binding.rpy_wall_matvec, binding.rpy_free_matvec):
+        full = fn(pos, lam)
+        halves = torch.cat([fn(pos, lam, rows=(0, n // 2)), fn(pos, lam, rows=(n // 2, n - n // 2))], dim=1)
+        e = rel_l2(full.cpu().numpy().astype(np.float64), halves.cpu().numpy().astype(np.float64))
+        print(f"symmetric vs plain kernel, {prec}: rel-L2 {e:.3e}")
+        assert e <= (1e-13 if prec == "f64" else 2e-6)
+        # the symmetric path is reproducible to rounding of the fp64 atomics, not bit for bit
+        again = fn(pos, lam)
+        assert rel_l2(again.cpu().numpy().astype(np.float64), full.cpu().numpy().astype(np.float64)) <= 1e-14
+
+
 # ------------------------------------------------------------------ degenerate cases
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_single_blob_and_coincident_blobs(prec):
