@@ -182,6 +182,35 @@ def make(config: int, **kw) -> Workload:
     return CONFIGS[config](**kw)
 
 
+@dataclass
+class Bodies:
+    """Rigid-body view of a workload: body p owns the contiguous blobs
+    offsets[p] .. offsets[p+1]-1 and has the tracking point q[p]; F are applied forces/torques."""
+    offsets: np.ndarray        # [n_bodies+1] int64
+    q: np.ndarray              # [n_bodies,3] float64
+    F: np.ndarray              # [n_bodies,6] float64 (f_p, tau_p), N(0,1)
+
+    @property
+    def n_bodies(self) -> int:
+        return int(self.q.shape[0])
+
+
+def bodies_of(w: Workload, seed: int = 1) -> Bodies:
+    """Bodies of a rigid-body workload (configs 2, 3, 5).  Tracking point q_p: the first blob of
+    the body (the boomerang's corner blob, config 2) / the mean of the body's blobs (the shell
+    centre, configs 3 and 5).  F ~ N(0,1)[nb,6] comes from its own generator (`seed`), so the blob
+    forces of the matvec workloads are unchanged."""
+    bpb = w.blobs_per_body
+    if bpb <= 1 or w.n_blobs % bpb:
+        raise ValueError("workload has no rigid bodies")
+    nb = w.n_blobs // bpb
+    offsets = np.arange(nb + 1, dtype=np.int64) * bpb
+    body = w.pos.reshape(nb, bpb, 3)
+    q = body[:, 0, :].copy() if w.name.startswith("cfg2") else body.mean(axis=1)
+    F = np.random.default_rng(seed).standard_normal((nb, 6))
+    return Bodies(offsets, q, F)
+
+
 def sample_rows(n: int, n_rows: int, seed: int = 12345) -> np.ndarray:
     """Seeded sorted sample of target rows used for parity / oracle timing at large N."""
     if n_rows >= n:

@@ -1,0 +1,123 @@
+"""Pins for oracle/rigid.py (the rigid-multiblob layer: K, Eq. (11), Eq. (12), Eq. (19)).
+
+None of these calls the oracle to check the oracle: printed values of the paper (Table I),
+hand-computed entries, identities re-evaluated term by term, and a textbook special case.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import rigid
+from paper_1602_02170_b200 import workloads
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+SIXPI = 6.0 * np.pi
+
+
+def _small_suspension(n_bodies=4, seed=3):
+    w = workloads.config2(seed=seed, n_bodies=n_bodies)
+    return w, workloads.bodies_of(w)
+
+
+def test_k_entries_by_hand():
+    """Eq. (2): r' = u + omega x (r - q)."""
+    pos = np.array([[2.0, 1.0, 5.0], [1.0, 3.0, 5.0]])
+    q = np.array([[1.0, 1.0, 5.0]])
+    off = np.array([0, 2])
+    # rotation about z with unit rate: the blob at q + (1,0,0) moves in +y, the one at q + (0,2,0) in -x
+    v = rigid.K_apply(pos, q, off, np.array([[0, 0, 0, 0, 0, 1.0]]))
+    assert np.allclose(v, [[0, 1, 0], [-2, 0, 0]])
+    v = rigid.K_apply(pos, q, off, np.array([[0.5, -1, 2, 0, 0, 0.0]]))
+    assert np.allclose(v, [[0.5, -1, 2], [0.5, -1, 2]])
+    # Eq. (10): a force (0, 1, 0) on the first blob gives torque (1,0,0) x (0,1,0) = +z about q
+    FT = rigid.KT_apply(pos, q, off, np.array([[0, 1.0, 0], [0, 0, 0]]))
+    assert np.allclose(FT, [[0, 1, 0, 0, 0, 1]])
+
+
+def test_kt_is_the_adjoint_of_k_and_rigid_motion_preserves_distances():
+    w, b = _small_suspension()
+    rng = np.random.default_rng(0)
+    U = rng.standard_normal((b.n_bodies, 6)); lam = rng.standard_normal(w.pos.shape)
+    lhs = np.sum(rigid.K_apply(w.pos, b.q, b.offsets, U) * lam)
+    rhs = np.sum(U * rigid.KT_apply(w.pos, b.q, b.offsets, lam))
+    assert lhs == pytest.approx(rhs, rel=1e-13)
+    K = rigid.K_matrix(w.pos, b.q, b.offsets)
+    assert np.allclose(K.T @ lam.reshape(-1), rigid.KT_apply(w.pos, b.q, b.offsets, lam).reshape(-1), atol=1e-12)
+    # rigid: relative velocity of two blobs of one body is perpendicular to their separation
+    v = rigid.K_apply(w.pos, b.q, b.offsets, U)
+    i, j = b.offsets[1], b.offsets[1] + 9
+    assert abs(np.dot(v[i] - v[j], w.pos[i] - w.pos[j])) < 1e-12
+
+
+def test_table1_effective_radii_through_body_mobility():
+    """Table I (left), through rigid.body_mobility and through the saddle-point
+    solve (11): an isolated shell pulled with force f moves with u = f / (6 pi eta R_h)."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "table1_radii.txt")) if l.strip() and l[0] != "#"]
+    for nb, a_over_s, rh_exp, rt_exp in rows:
+        pos = workloads.shell_template(int(nb))
+        d = np.linalg.norm(pos[:, None] - pos[None], axis=2)
+        a = float(a_over_s) * d[d > 1e-9].min()
+        off = np.array([0, pos.shape[0]]); q = np.zeros((1, 3))
+        N = rigid.body_mobility(oracle.FREE, pos, q, off, a, 1.0)
+        assert 1.0 / (SIXPI * np.trace(N[:3, :3]) / 3) == pytest.approx(float(rh_exp), abs=1.5e-4)
+        assert (1.0 / (8 * np.pi * np.trace(N[3:, 3:]) / 3)) ** (1 / 3) == pytest.approx(float(rt_exp), abs=1.5e-4)
+        lam, U = rigid.mobility_solve(oracle.FREE, pos, q, off, np.array([[1.0, 0, 0, 0, 0, 0]]), None, a, 1.0)
+        assert U[0, 0] == pytest.approx(1.0 / (SIXPI * float(rh_exp)), rel=2e-4)
+        assert np.allclose(U[0, 1:], 0, atol=1e-9)          # icosahedral symmetry: no coupling
+        assert np.allclose(lam.sum(axis=0), [1, 0, 0], atol=1e-12)
+
+
+@pytest.mark.parametrize("variant", [oracle.FREE, oracle.WALL])
+def test_mobility_solve_satisfies_eq10_term_by_term(variant):
+    """The three equations of (10), re-evaluated with the matvec oracle (row
+    loop, not the dense assembly) and explicit cross products."""
+    w, b = _small_suspension(n_bodies=5)
+    rng = np.random.default_rng(1)
+    slip = 0.1 * rng.standard_normal(w.pos.shape)
+    lam, U = rigid.mobility_solve(variant, w.pos, b.q, b.offsets, b.F, slip, 1.0, 1.0)
+    Ml = oracle.matvec(variant, w.pos, lam)
+    for p in range(b.n_bodies):
+        f = np.zeros(3); t = np.zeros(3)
+        for i in range(b.offsets[p], b.offsets[p + 1]):
+            rhs = U[p, :3] + np.cross(U[p, 3:], w.pos[i] - b.q[p]) + slip[i]
+            assert np.allclose(Ml[i], rhs, atol=1e-10)
+            f += lam[i]; t += np.cross(w.pos[i] - b.q[p], lam[i])
+        assert np.allclose(f, b.F[p, :3], atol=1e-10) and np.allclose(t, b.F[p, 3:], atol=1e-10)
+
+
+def test_body_mobility_is_spd_and_wall_slows_the_body():
+    w, b = _small_suspension(n_bodies=3)
+    for variant in (oracle.FREE, oracle.WALL):
+        N = rigid.body_mobility(variant, w.pos, b.q, b.offsets)
+        assert np.allclose(N, N.T, atol=1e-12)
+        assert np.linalg.eigvalsh(N).min() > 0          # PAPER.md:177 "evidently SPD since M is"
+    # one shell: the wall reduces the translational mobility (Fig. 5)
+    pos = 3.0 * workloads.shell_template(42) + np.array([0, 0, 4.5])
+    off = np.array([0, 42]); q = np.array([[0, 0, 4.5]])
+    Nf = rigid.body_mobility(oracle.FREE, pos, q, off); Nw = rigid.body_mobility(oracle.WALL, pos, q, off)
+    assert 0.3 * Nf[0, 0] < Nw[0, 0] < 0.9 * Nf[0, 0] and Nw[2, 2] < Nw[0, 0]
+
+
+def test_preconditioner_is_exact_for_one_body_and_block_diagonal_otherwise():
+    """Eq. (17)-(19)."""
+    w, b = _small_suspension(n_bodies=1)
+    rng = np.random.default_rng(2)
+    x = rng.standard_normal(w.pos.shape)
+    lam, U = rigid.precond_solve(oracle.WALL, w.pos, b.q, b.offsets, x, -b.F)
+    lam2, U2 = rigid.mobility_solve(oracle.WALL, w.pos, b.q, b.offsets, b.F, x)
+    assert np.allclose(lam, lam2, atol=1e-10) and np.allclose(U, U2, atol=1e-10)
+    # several bodies: the solve of body p ignores every other body's blobs
+    w, b = _small_suspension(n_bodies=3)
+    x = rng.standard_normal(w.pos.shape)
+    lam, U = rigid.precond_solve(oracle.WALL, w.pos, b.q, b.offsets, x, -b.F)
+    s = slice(b.offsets[1], b.offsets[2])
+    lam1, U1 = rigid.mobility_solve(oracle.WALL, w.pos[s], b.q[1:2], np.array([0, 15]), b.F[1:2], x[s])
+    assert np.allclose(lam[s], lam1, atol=1e-10) and np.allclose(U[1], U1[0], atol=1e-10)
+    # residual of (19) with the block-diagonal M~ assembled from body_blocks
+    blocks = rigid.body_blocks(oracle.WALL, w.pos, b.offsets)
+    for p, Mpp in enumerate(blocks):
+        sp = slice(b.offsets[p], b.offsets[p + 1])
+        r = Mpp @ lam[sp].reshape(-1) - rigid.K_apply(w.pos[sp], b.q[p:p + 1], np.array([0, 15]), U[p:p + 1]).reshape(-1)
+        assert np.allclose(r, x[sp].reshape(-1), atol=1e-10)
