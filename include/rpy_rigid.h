@@ -1,0 +1,132 @@
+/*
+ * rpy_rigid.h -- C ABI of the rigid-multiblob layer around the mobility matvec (SURVEY.md 8(f)
+ * rows N1, N2): the kinematic matrix K and its transpose, the block-diagonal preconditioner, and
+ * the preconditioned GMRES solve of the mobility problem.  Same library as rpy_matvec.h
+ * (librpy_matvec.so), same conventions: plain device / host pointers, no allocation, no state,
+ * errors as return codes, sm_100a only, no CPU fallback.
+ *
+ * The operations (arXiv:1602.02170; line numbers are /root/reference/PAPER.md):
+ *
+ *   K U         blob velocities of rigid motion, (K U)_i = u_p + omega_p x (r_i - q_p) for the blobs
+ *               i of body p                                               Eqs. (2)-(3)
+ *   K^T lambda  total force and torque per body, f_p = sum_i lambda_i,
+ *               tau_p = sum_i (r_i - q_p) x lambda_i                       Eq. (10)
+ *   P^-1        the indefinite block-diagonal preconditioner of Eq. (18): solve Eq. (19),
+ *               [M~ -K; -K^T 0][lambda; U] = [x; y], with M~ the diagonal blocks M^(pp) of Eq. (17)
+ *               (each body alone, with or without the wall), through a dense Cholesky
+ *               factorisation of every M^(pp) and the 6x6 body mobilities
+ *               N~_pp = (K_p^T (M^(pp))^-1 K_p)^-1
+ *   solve       Eq. (11), [M -K; -K^T 0][lambda; U] = [slip; -F], by right-preconditioned
+ *               restarted GMRES
+ *
+ * Bodies are contiguous runs of blobs: body p owns blobs offsets[p] .. offsets[p+1]-1
+ * (offsets[0] = 0, offsets[n_bodies] = n_blobs, every body has >= 1 blob and at most
+ * RPY_RIGID_MAX_BODY_BLOBS) and has the tracking point q[p].  Rigid motions and force/torque pairs
+ * are stored [n_bodies][6] = (u_p, omega_p) / (f_p, tau_p).  A solver vector is the concatenation
+ * [lambda (3 n_blobs doubles, blob-major) ; U (6 n_bodies doubles)].
+ *
+ * Everything in this header is double precision, except that the solve can run its O(N^2) matvec
+ * through the fp32 path of rpy_matvec.h (matvec_prec = RPY_PREC_F32_ACC64: the iterate is rounded
+ * to float for the product and the residual stalls near 1e-6; "single precision can be used for
+ * lower accuracy requirements").
+ */
+#ifndef RPY_RIGID_H
+#define RPY_RIGID_H
+
+#include "rpy_matvec.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RPY_RIGID_MAX_BODY_BLOBS 512
+#define RPY_RIGID_MAX_RESTART 128
+
+/* Additional status (values continue rpy_status): the Cholesky factorisation of some M^(pp) met a
+ * non-positive pivot (a blob overlapping the wall, or coincident blobs). */
+#define RPY_ERR_NOT_SPD 6
+
+/* out[i] = beta * out[i] + alpha * (K U)_i.   beta == 0 overwrites (out may be uninitialised).
+ *   d_pos [n_blobs][3], d_q [n_bodies][3], d_offsets [n_bodies+1] (int64), d_U [n_bodies][6],
+ *   d_out [n_blobs][3] : device.  One warp per body.                                              */
+rpy_status rpy_rigid_K_apply(int64_t n_blobs, int64_t n_bodies, const double *d_pos, const double *d_q,
+                             const int64_t *d_offsets, const double *d_U, double alpha, double beta,
+                             double *d_out, void *cuda_stream);
+
+/* out[p] = beta * out[p] + alpha * (K^T lambda)_p;  d_lambda [n_blobs][3], d_out [n_bodies][6].
+ * One warp per body, fixed summation order (bit-reproducible).                                    */
+rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double *d_pos, const double *d_q,
+                              const int64_t *d_offsets, const double *d_lambda, double alpha, double beta,
+                              double *d_out, void *cuda_stream);
+
+/* Bytes of device memory the preconditioner of these bodies needs (host arithmetic on the HOST
+ * array h_offsets [n_bodies+1]); 0 if the offsets are not a valid partition.  Per body with
+ * m = 3 * blobs: m*m doubles (Cholesky factor L in the lower triangle AND L^T in the upper one, so
+ * both substitutions read contiguous rows), m*6 (Y = (M^(pp))^-1 K_p), 36 (N~_pp), plus tables.  */
+size_t rpy_rigid_precond_bytes(int64_t n_bodies, const int64_t *h_offsets);
+
+/* Builds the preconditioner: for every body the dense M^(pp) (wall != 0: wall-corrected tensor,
+ * else free space -- the "unbounded" preconditioner of Table III), its Cholesky
+ * factor, Y and N~_pp.  One CTA per body; the matrix lives in shared memory when 3*blobs <= 162,
+ * else in its slot of d_precond.  h_offsets is read before the call returns.
+ * d_precond: device, 256-byte aligned, >= rpy_rigid_precond_bytes().  Synchronises the stream once (after
+ * copying the offset tables up, before the build kernel is enqueued); a failed
+ * factorisation is recorded in d_precond and reported by rpy_rigid_precond_info / the solve.     */
+rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, const double *d_pos,
+                                   const double *d_q, const int64_t *h_offsets, double a, double eta,
+                                   void *d_precond, size_t precond_bytes, void *cuda_stream);
+
+/* Synchronises the stream and writes to *h_first_bad_body the smallest body index whose
+ * factorisation failed, or -1.  Returns RPY_ERR_NOT_SPD in the former case.                        */
+rpy_status rpy_rigid_precond_info(int64_t n_bodies, const void *d_precond, int64_t *h_first_bad_body,
+                                  void *cuda_stream);
+
+/* [lambda; U] = P^-1 [x; y]: Eq. (19) for every body.  d_in, d_out: solver vectors
+ * (3 n_blobs + 6 n_bodies doubles), d_out must not overlap d_in.  One warp per body:
+ * t = (M^(pp))^-1 x by two triangular substitutions, U = -N~ (y + Y^T x), lambda = t + Y U.      */
+rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void *d_precond,
+                                   const double *d_in, double *d_out, void *cuda_stream);
+
+/* Copies out pieces of a built preconditioner (tests, diagnostics): for body p, the factor
+ * (row-major m x m, L in the lower triangle, L^T mirrored above) to d_factor if non-NULL, and the
+ * 6x6 N~_pp (row-major) to d_body_mobility if non-NULL.  Device to device, stream ordered.        */
+rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t *h_offsets, const void *d_precond,
+                                 int64_t body, double *d_factor, double *d_body_mobility,
+                                 void *cuda_stream);
+
+/* Workspace of the solve: restart+1 Krylov vectors, three work vectors, the matvec workspace and
+ * (fp32 matvec) float copies of positions, iterate and product.                                   */
+size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart);
+
+/* Solves the mobility problem, Eq. (11), for lambda and U given the applied forces/torques F and an
+ * optional slip velocity, by right-preconditioned GMRES(restart) from a zero initial guess: the
+ * iteration stops when the residual of (11) is <= tol * ||[slip; -F]|| (Table III: tol = 1e-8,
+ * PAPER.md:680) or after max_iter matrix applications.  One iteration = P^-1 (above), the O(N^2)
+ * product M lambda (rpy_wall_matvec / rpy_free_matvec with matvec_prec), K, K^T, classical
+ * Gram-Schmidt applied twice, and a Givens update of the small Hessenberg problem -- all on the
+ * device; the host reads one double (the residual norm) per iteration, so the call SYNCHRONISES.
+ *   wall        != 0: wall-corrected M in the product (the preconditioner is whatever was built)
+ *   d_F         [n_bodies][6] device;  d_slip [n_blobs][3] device or NULL (zero slip)
+ *   d_lambda    [n_blobs][3], d_U [n_bodies][6] : device, overwritten
+ *   h_history   host, max_iter+1 doubles or NULL: relative residual after each iteration, [0] = 1
+ *   h_n_iter    host, matrix applications used;  h_rel_resid host, final relative residual estimate
+ * Returns RPY_OK also when max_iter was reached without convergence (check *h_rel_resid).         */
+rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
+                                    const double *d_pos, const double *d_q, const int64_t *d_offsets,
+                                    const double *d_F, const double *d_slip, double a, double eta,
+                                    const void *d_precond, double tol, int restart, int max_iter,
+                                    double *d_lambda, double *d_U,
+                                    double *h_history, int *h_n_iter, double *h_rel_resid,
+                                    void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* The operator of Eq. (11) alone: out = [M lambda - K U ; -K^T lambda] for a solver vector
+ * in = [lambda; U] (tests; residual checks).  d_workspace as for the solve with restart = 1.      */
+rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
+                                  const double *d_pos, const double *d_q, const int64_t *d_offsets,
+                                  double a, double eta, const double *d_in, double *d_out,
+                                  void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RPY_RIGID_H */

@@ -16,8 +16,9 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "librpy_matvec.so"
-SOURCES = [CSRC / "rpy_matvec.cu", CSRC / "rpy_probe.cu"]
-DEPS = SOURCES + [CSRC / "rpy_math.cuh", CSRC / "rpy_kernels.cuh", INCLUDE / "rpy_matvec.h"]
+SOURCES = [CSRC / "rpy_matvec.cu", CSRC / "rpy_probe.cu", CSRC / "rpy_rigid.cu"]
+DEPS = SOURCES + [CSRC / "rpy_math.cuh", CSRC / "rpy_kernels.cuh", CSRC / "rpy_internal.h",
+               INCLUDE / "rpy_matvec.h", INCLUDE / "rpy_rigid.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

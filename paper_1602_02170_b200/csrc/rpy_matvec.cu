@@ -7,6 +7,7 @@
 #include <stddef.h>
 #include "../../include/rpy_matvec.h"
 #include "rpy_kernels.cuh"
+#include "rpy_internal.h"
 
 #ifndef RPY_SYM_MINB_F32
 #define RPY_SYM_MINB_F32 3
@@ -352,6 +353,10 @@ rpy_status matvec_host(bool wall, rpy_prec prec, int64_t n, int n_rhs, const voi
 }
 
 }  // namespace
+
+namespace rpy {
+rpy_status set_cuda_error(cudaError_t e) { return cuda_fail(e); }
+}  // namespace rpy
 
 extern "C" {
 

@@ -1,0 +1,928 @@
+// rpy_rigid.cu -- the rigid-multiblob layer of include/rpy_rigid.h: K, K^T (Eqs. (2)-(3), (10)),
+// the block-diagonal preconditioner of Eqs. (17)-(19) (dense per-body M^(pp), Cholesky, N~_pp) and
+// right-preconditioned GMRES on the saddle-point system (11).  arXiv:1602.02170 Section II
+// (PAPER.md:79-84, 154-252).  sm_100a only; no allocation, no state.
+//
+// Kernels:
+//   k_apply / kt_apply        one warp per body; O(N_b)
+//   precond_build             one CTA per body: dense M^(pp) from the same pair arithmetic as the
+//                             matvec (rpy_math.cuh, double lanes), in-place Cholesky, Y = M^-1 K,
+//                             N~ = (K^T Y)^-1
+//   precond_apply             one warp per body: two triangular substitutions + 6x6 work
+//   dots / update / hessenberg / scale / combine      the Krylov vector operations of GMRES
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/rpy_rigid.h"
+#include "rpy_math.cuh"
+#include "rpy_internal.h"
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr int kSmemBodyM = 162;            // largest 3*blobs whose matrix is factorised in shared memory
+constexpr int kBuildThreads = 256;
+constexpr int64_t kMagic = 0x52505952494744LL;   // "RPYRIGD"
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline rpy_status st_of(int s) { return static_cast<rpy_status>(s); }
+
+// ------------------------------------------------------------------ K and K^T
+// (K U)_i = u_p + omega_p x (r_i - q_p), Eq. (2).
+__global__ void k_apply_kernel(const double* __restrict__ pos, const double* __restrict__ q,
+                               const int64_t* __restrict__ offsets, const double* __restrict__ U,
+                               double alpha, double beta, double* __restrict__ out, int64_t n_bodies)
+{
+    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (p >= n_bodies) return;
+    const double ux = U[6 * p + 0], uy = U[6 * p + 1], uz = U[6 * p + 2];
+    const double wx = U[6 * p + 3], wy = U[6 * p + 4], wz = U[6 * p + 5];
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    for (int64_t i = offsets[p] + lane; i < offsets[p + 1]; i += 32) {
+        const double dx = pos[3 * i + 0] - qx, dy = pos[3 * i + 1] - qy, dz = pos[3 * i + 2] - qz;
+        const double vx = ux + (wy * dz - wz * dy);
+        const double vy = uy + (wz * dx - wx * dz);
+        const double vz = uz + (wx * dy - wy * dx);
+        if (beta == 0.0) {
+            out[3 * i + 0] = alpha * vx; out[3 * i + 1] = alpha * vy; out[3 * i + 2] = alpha * vz;
+        } else {
+            out[3 * i + 0] = beta * out[3 * i + 0] + alpha * vx;
+            out[3 * i + 1] = beta * out[3 * i + 1] + alpha * vy;
+            out[3 * i + 2] = beta * out[3 * i + 2] + alpha * vz;
+        }
+    }
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// f_p = sum lambda_i, tau_p = sum (r_i - q_p) x lambda_i, Eq. (10).
+__global__ void kt_apply_kernel(const double* __restrict__ pos, const double* __restrict__ q,
+                                const int64_t* __restrict__ offsets, const double* __restrict__ lam,
+                                double alpha, double beta, double* __restrict__ out, int64_t n_bodies)
+{
+    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (p >= n_bodies) return;
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int64_t i = offsets[p] + lane; i < offsets[p + 1]; i += 32) {
+        const double dx = pos[3 * i + 0] - qx, dy = pos[3 * i + 1] - qy, dz = pos[3 * i + 2] - qz;
+        const double lx = lam[3 * i + 0], ly = lam[3 * i + 1], lz = lam[3 * i + 2];
+        s[0] += lx; s[1] += ly; s[2] += lz;
+        s[3] += dy * lz - dz * ly;
+        s[4] += dz * lx - dx * lz;
+        s[5] += dx * ly - dy * lx;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) s[c] = warp_sum(s[c]);
+    if (lane < 6) {
+        double v = s[0];
+#pragma unroll
+        for (int c = 1; c < 6; ++c) if (lane == c) v = s[c];
+        out[6 * p + lane] = (beta == 0.0 ? 0.0 : beta * out[6 * p + lane]) + alpha * v;
+    }
+}
+
+// ------------------------------------------------------------------ preconditioner storage
+// [header 4 x int64][offsets nb+1][mat_off nb+1][info nb x int32][factors][Y 3N x 6][Nt nb x 36]
+struct PrecondLayout {
+    size_t offsets_at, matoff_at, info_at, factors_at, y_at, nt_at, total;
+    int64_t n_blobs, total_mat;
+    int max_m;
+};
+
+bool layout_of(int64_t nb, const int64_t* h_off, PrecondLayout& L)
+{
+    if (nb < 1 || !h_off || h_off[0] != 0) return false;
+    int64_t tot = 0; int max_m = 0;
+    for (int64_t p = 0; p < nb; ++p) {
+        int64_t c = h_off[p + 1] - h_off[p];
+        if (c < 1 || c > RPY_RIGID_MAX_BODY_BLOBS) return false;
+        tot += 9 * c * c;
+        if (3 * c > max_m) max_m = (int)(3 * c);
+    }
+    L.n_blobs = h_off[nb]; L.total_mat = tot; L.max_m = max_m;
+    size_t at = align_up(4 * sizeof(int64_t), kAlign);
+    L.offsets_at = at; at = align_up(at + (size_t)(nb + 1) * 8, kAlign);
+    L.matoff_at = at;  at = align_up(at + (size_t)(nb + 1) * 8, kAlign);
+    L.info_at = at;    at = align_up(at + (size_t)nb * 4, kAlign);
+    L.factors_at = at; at = align_up(at + (size_t)tot * 8, kAlign);
+    L.y_at = at;       at = align_up(at + (size_t)L.n_blobs * 18 * 8, kAlign);
+    L.nt_at = at;      at = align_up(at + (size_t)nb * 36 * 8, kAlign);
+    L.total = at;
+    return true;
+}
+
+// Device-side view rebuilt from (n_blobs, n_bodies, total_mat) without the host offsets.
+struct PrecondView {
+    const int64_t* offsets; const int64_t* mat_off; int* info; double* factors; double* Y; double* Nt;
+};
+__host__ __device__ inline size_t align_up_hd(size_t x) { return (x + 255) / 256 * 256; }
+// header: [0] magic, [1] n_bodies, [2] n_blobs, [3] total_mat (doubles in the factor region)
+__host__ __device__ inline PrecondView view_of(void* base, int64_t nb, int64_t n_blobs, int64_t total_mat)
+{
+    unsigned char* b = static_cast<unsigned char*>(base);
+    size_t at = align_up_hd(4 * sizeof(int64_t));
+    PrecondView v;
+    v.offsets = reinterpret_cast<const int64_t*>(b + at); at = align_up_hd(at + (size_t)(nb + 1) * 8);
+    v.mat_off = reinterpret_cast<const int64_t*>(b + at); at = align_up_hd(at + (size_t)(nb + 1) * 8);
+    v.info = reinterpret_cast<int*>(b + at);              at = align_up_hd(at + (size_t)nb * 4);
+    v.factors = reinterpret_cast<double*>(b + at);        at = align_up_hd(at + (size_t)total_mat * 8);
+    v.Y = reinterpret_cast<double*>(b + at);              at = align_up_hd(at + (size_t)n_blobs * 18 * 8);
+    v.Nt = reinterpret_cast<double*>(b + at);
+    return v;
+}
+
+// ------------------------------------------------------------------ dense 3x3 block (double lanes)
+// The block M_ij * (6 pi eta a) from the matvec's own pair arithmetic: the five collected scalars of
+// rpy_math.cuh give  [al + be dx dx, be dx dy, ga dx; be dx dy, al + be dy dy, ga dy; ep dx, ep dy, de]
+// (wall) or f I + G d d^T (free).  Positions are already divided by a.
+template <bool WALL>
+__device__ __forceinline__ void pair_block(double xi, double yi, double zi, double xj, double yj, double zj,
+                                           double B[9])
+{
+    using L = rpy::Lane<double>;
+    rpy::PairCoef<double> c;
+    c.dx = xi - xj; c.dy = yi - yj; c.dz = zi - zj;
+    double rxy2, r2, f, G;
+    rpy::rpy_far_scalars<L>(c.dx, c.dy, c.dz, rxy2, r2, f, G);
+    if (r2 <= 4.0) rpy::rpy_near_fixup<L>(r2, f, G);
+    if (WALL) {
+        rpy::wall_coef<L>(zi, zj, rxy2, f, G, c);
+        B[0] = c.al + c.be * c.dx * c.dx; B[1] = c.be * c.dx * c.dy;        B[2] = c.ga * c.dx;
+        B[3] = B[1];                      B[4] = c.al + c.be * c.dy * c.dy; B[5] = c.ga * c.dy;
+        B[6] = c.ep * c.dx;               B[7] = c.ep * c.dy;               B[8] = c.de;
+    } else {
+        B[0] = f + G * c.dx * c.dx; B[1] = G * c.dx * c.dy;     B[2] = G * c.dx * c.dz;
+        B[3] = B[1];                B[4] = f + G * c.dy * c.dy; B[5] = G * c.dy * c.dz;
+        B[6] = B[2];                B[7] = B[5];                B[8] = f + G * c.dz * c.dz;
+    }
+}
+
+// ------------------------------------------------------------------ preconditioner build
+// One CTA per body.  A (m x m, leading dimension ld) is in shared memory when m <= kSmemBodyM, else
+// it is the body's slot of `factors` (ld = m).  Steps: fill M^(pp); right-looking Cholesky on the
+// lower triangle, one barrier per column (thread t owns trailing columns k = j+1+t, ...: its
+// multiplier A[k][j] stays in a register, A[i][j] is a broadcast read, A[i][k] is conflict-free /
+// coalesced across threads); Y = (L L^T)^-1 K_p, one warp per column of K_p; N~ = (K_p^T Y)^-1 by
+// Gauss-Jordan on the 6x6; store L mirrored into both triangles.
+template <bool WALL>
+__global__ void __launch_bounds__(kBuildThreads)
+precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ q,
+                     const int64_t* __restrict__ offsets, const int64_t* __restrict__ mat_off,
+                     int* __restrict__ info, double* __restrict__ factors, double* __restrict__ Yg,
+                     double* __restrict__ Ntg, double inv_a, double scale)
+{
+    extern __shared__ __align__(16) double sm[];
+    __shared__ double s_n[36];
+    __shared__ int s_fail;
+    const int p = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t b0 = offsets[p];
+    const int nbp = (int)(offsets[p + 1] - b0);
+    const int m = 3 * nbp;
+    const bool in_smem = m <= kSmemBodyM;
+    double* const G = factors + mat_off[p];
+    const int ld = in_smem ? (m | 1) : m;
+    double* const A = in_smem ? sm : G;
+    double* const Yb = in_smem ? sm + (size_t)ld * m : Yg + b0 * 18;      // [m][6]
+    if (tid == 0) s_fail = 0;
+
+    for (int e = tid; e < nbp * nbp; e += kBuildThreads) {
+        const int bi = e / nbp, bj = e % nbp;
+        const double* ri = pos + 3 * (b0 + bi);
+        const double* rj = pos + 3 * (b0 + bj);
+        double B[9];
+        pair_block<WALL>(ri[0] * inv_a, ri[1] * inv_a, ri[2] * inv_a, rj[0] * inv_a, rj[1] * inv_a, rj[2] * inv_a, B);
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) A[(size_t)(3 * bi + r) * ld + 3 * bj + c] = scale * B[3 * r + c];
+    }
+    __syncthreads();
+
+    for (int j = 0; j < m; ++j) {
+        const double d = A[(size_t)j * ld + j];
+        if (!(d > 0.0) || !isfinite(d)) { if (tid == 0) s_fail = j + 1; break; }   // uniform: all threads read the same d
+        const double rd = 1.0 / d;
+        for (int k = j + 1 + tid; k < m; k += kBuildThreads) {
+            const double ckj = A[(size_t)k * ld + j] * rd;
+            for (int i = k; i < m; ++i) A[(size_t)i * ld + k] -= A[(size_t)i * ld + j] * ckj;
+        }
+        __syncthreads();
+        const double rs = 1.0 / sqrt(d);
+        for (int i = j + tid; i < m; i += kBuildThreads)
+            A[(size_t)i * ld + j] = i == j ? sqrt(d) : A[(size_t)i * ld + j] * rs;
+    }
+    __syncthreads();
+    if (s_fail) {
+        if (tid == 0) info[p] = s_fail;
+        return;
+    }
+
+    // K_p rows of blob i (real lengths): [I | C_i], C_i = [[0, dz, -dy], [-dz, 0, dx], [dy, -dx, 0]]
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    auto k_entry = [&](int row, int col) -> double {
+        const int i = row / 3, r = row % 3;
+        if (col < 3) return r == col ? 1.0 : 0.0;
+        const double* ri = pos + 3 * (b0 + i);
+        const double dx = ri[0] - qx, dy = ri[1] - qy, dz = ri[2] - qz;
+        const int c = col - 3;
+        if (r == c) return 0.0;
+        if (r == 0) return c == 1 ? dz : -dy;
+        if (r == 1) return c == 0 ? -dz : dx;
+        return c == 0 ? dy : -dx;
+    };
+    if (warp < 6) {
+        const int c = warp;
+        for (int i = lane; i < m; i += 32) Yb[(size_t)i * 6 + c] = k_entry(i, c);
+        __syncwarp();
+        for (int j = 0; j < m; ++j) {                       // L y = k
+            const double yj = Yb[(size_t)j * 6 + c] / A[(size_t)j * ld + j];
+            __syncwarp();
+            if (lane == 0) Yb[(size_t)j * 6 + c] = yj;
+            for (int i = j + 1 + lane; i < m; i += 32) Yb[(size_t)i * 6 + c] -= A[(size_t)i * ld + j] * yj;
+            __syncwarp();
+        }
+        for (int j = m - 1; j >= 0; --j) {                  // L^T x = y
+            const double xj = Yb[(size_t)j * 6 + c] / A[(size_t)j * ld + j];
+            __syncwarp();
+            if (lane == 0) Yb[(size_t)j * 6 + c] = xj;
+            for (int i = lane; i < j; i += 32) Yb[(size_t)i * 6 + c] -= A[(size_t)j * ld + i] * xj;
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    if (tid < 36) {
+        const int r = tid / 6, c = tid % 6;
+        double s = 0.0;
+        for (int i = 0; i < m; ++i) s += k_entry(i, r) * Yb[(size_t)i * 6 + c];
+        s_n[tid] = s;
+    }
+    __syncthreads();
+    if (tid == 0) {                                          // invert the SPD 6x6 (Gauss-Jordan, no pivoting needed)
+        double a[6][12];
+        for (int r = 0; r < 6; ++r)
+            for (int c = 0; c < 6; ++c) { a[r][c] = 0.5 * (s_n[6 * r + c] + s_n[6 * c + r]); a[r][6 + c] = r == c ? 1.0 : 0.0; }
+        bool ok = true;
+        for (int k = 0; k < 6; ++k) {
+            const double piv = a[k][k];
+            if (!(piv > 0.0) || !isfinite(piv)) { ok = false; break; }
+            const double rp = 1.0 / piv;
+            for (int c = 0; c < 12; ++c) a[k][c] *= rp;
+            for (int r = 0; r < 6; ++r) {
+                if (r == k) continue;
+                const double fct = a[r][k];
+                for (int c = 0; c < 12; ++c) a[r][c] -= fct * a[k][c];
+            }
+        }
+        for (int r = 0; r < 6; ++r)
+            for (int c = 0; c < 6; ++c) Ntg[(size_t)p * 36 + 6 * r + c] = ok ? a[r][6 + c] : 0.0;
+        info[p] = ok ? 0 : m + 1;
+    }
+    // store: S[i][j] = S[j][i] = L[max][min]; Y rows
+    for (int e = tid; e < m * m; e += kBuildThreads) {
+        const int i = e / m, j = e % m;
+        const int hi = i > j ? i : j, lo = i > j ? j : i;
+        if (in_smem) G[e] = A[(size_t)hi * ld + lo];
+        else if (j > i) G[e] = A[(size_t)hi * ld + lo];      // mirror the lower triangle upwards in place
+    }
+    if (in_smem)
+        for (int e = tid; e < m * 6; e += kBuildThreads) Yg[b0 * 18 + e] = Yb[e];
+}
+
+// ------------------------------------------------------------------ preconditioner apply
+// One warp per body: [lambda; U] = P_p^-1 [x; y] (Eq. (19)):
+//   r = Y^T x (= K^T M^-1 x),  U = -N~ (y + r),  t = M^-1 x by L t' = x, L^T t = t',  lambda = t + Y U.
+// The right-hand side lives in the warp's slice of `out` (each warp touches only its own body's
+// entries); row j of the stored factor holds column j of L to the right of the diagonal and row j of
+// L to its left, so both substitutions read one contiguous row per step.
+__global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
+                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies)
+{
+    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    const int64_t* hdr = static_cast<const int64_t*>(precond);
+    if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
+    const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
+    const int64_t* offsets = pv.offsets;
+    const int64_t* mat_off = pv.mat_off;
+    const double* factors = pv.factors;
+    const double* Yg = pv.Y;
+    const double* Ntg = pv.Nt;
+    const int64_t b0 = offsets[p];
+    const int m = 3 * (int)(offsets[p + 1] - b0);
+    const double* S = factors + mat_off[p];
+    const double* Y = Yg + b0 * 18;
+    const double* x = in + 3 * b0;
+    const double* y = in + 3 * n_blobs + 6 * p;
+    double* t = out + 3 * b0;
+
+    double r[6] = {0, 0, 0, 0, 0, 0};
+    for (int i = lane; i < m; i += 32) {
+        const double xi = x[i];
+        t[i] = xi;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) r[c] += Y[(size_t)i * 6 + c] * xi;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) r[c] = warp_sum(r[c]) + y[c];
+    double U[6];
+#pragma unroll
+    for (int a = 0; a < 6; ++a) {
+        double s = 0.0;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) s += Ntg[(size_t)p * 36 + 6 * a + c] * r[c];
+        U[a] = -s;
+    }
+    __syncwarp();
+
+    // forward: for j = 0..m-1: t_j /= L_jj; t_i -= L_ij t_j (i > j); L_ij = S[j][i]
+    for (int j = 0; j < m; ++j) {
+        const double* row = S + (size_t)j * m;
+        const double tj = t[j] / row[j];
+        __syncwarp();
+        if (lane == 0) t[j] = tj;
+        for (int i = j + 1 + lane; i < m; i += 32) t[i] -= row[i] * tj;
+        __syncwarp();
+    }
+    // backward: for j = m-1..0: t_j /= L_jj; t_i -= L_ji t_j (i < j); L_ji = S[j][i]
+    for (int j = m - 1; j >= 0; --j) {
+        const double* row = S + (size_t)j * m;
+        const double tj = t[j] / row[j];
+        __syncwarp();
+        if (lane == 0) t[j] = tj;
+        for (int i = lane; i < j; i += 32) t[i] -= row[i] * tj;
+        __syncwarp();
+    }
+    for (int i = lane; i < m; i += 32) {
+        double s = t[i];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) s += Y[(size_t)i * 6 + c] * U[c];
+        t[i] = s;
+    }
+    if (lane < 6) {
+        double v = U[0];
+#pragma unroll
+        for (int c = 1; c < 6; ++c) if (lane == c) v = U[c];
+        out[3 * n_blobs + 6 * p + lane] = v;
+    }
+}
+
+// ------------------------------------------------------------------ Krylov vector operations
+// Vectors have n = 3 n_blobs + 6 n_bodies doubles.  A fixed grid of kVecBlocks CTAs cuts [0, n)
+// into equal contiguous chunks; every reduction is two-stage (per-CTA partials, then a fixed-order
+// sum), so the solve is bit-reproducible whenever the matvec is.
+constexpr int kVecBlocks = 296;       // 2 CTAs per SM
+constexpr int kVecThreads = 256;
+
+__device__ __forceinline__ void chunk_of(int64_t n, int64_t& lo, int64_t& hi)
+{
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    lo = (int64_t)blockIdx.x * per;
+    hi = lo + per < n ? lo + per : n;
+    if (lo > n) lo = n;
+}
+
+// partial[v * gridDim.x + blk] = sum over the CTA's chunk of V[v][i] * w[i], v = 0..nvec-1.
+// Warp w of the CTA takes v = w, w + 8, ...; no CTA barrier.
+__global__ void __launch_bounds__(kVecThreads)
+dots_kernel(const double* __restrict__ V, int64_t ldv, int nvec, const double* __restrict__ w, int64_t n,
+            double* __restrict__ partial)
+{
+    int64_t lo, hi; chunk_of(n, lo, hi);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int v = warp; v < nvec; v += kVecThreads / 32) {
+        const double* a = V + (int64_t)v * ldv;
+        double s = 0.0;
+        for (int64_t i = lo + lane; i < hi; i += 32) s += a[i] * w[i];
+        s = warp_sum(s);
+        if (lane == 0) partial[(int64_t)v * gridDim.x + blockIdx.x] = s;
+    }
+}
+
+// h[v] = sum_blk partial[v][blk] (fixed order);  w -= sum_v h[v] V[v];  norm_partial[blk] = |w chunk|^2;
+// CTA 0 also does hcol[v] = (accumulate ? hcol[v] : 0) + h[v].
+__global__ void __launch_bounds__(kVecThreads)
+update_kernel(const double* __restrict__ V, int64_t ldv, int nvec, double* __restrict__ w, int64_t n,
+              const double* __restrict__ partial, double* __restrict__ hcol, int accumulate,
+              double* __restrict__ norm_partial)
+{
+    __shared__ double h[RPY_RIGID_MAX_RESTART + 1];
+    __shared__ double red[kVecThreads / 32];
+    for (int v = threadIdx.x; v < nvec; v += kVecThreads) {
+        double s = 0.0;
+        for (int b = 0; b < (int)gridDim.x; ++b) s += partial[(int64_t)v * gridDim.x + b];
+        h[v] = s;
+        if (blockIdx.x == 0) hcol[v] = (accumulate ? hcol[v] : 0.0) + s;
+    }
+    __syncthreads();
+    int64_t lo, hi; chunk_of(n, lo, hi);
+    double nrm = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) {
+        double wi = w[i];
+        for (int v = 0; v < nvec; ++v) wi -= h[v] * V[(int64_t)v * ldv + i];
+        w[i] = wi;
+        nrm += wi * wi;
+    }
+    nrm = warp_sum(nrm);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = nrm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < kVecThreads / 32; ++k) s += red[k];
+        norm_partial[blockIdx.x] = s;
+    }
+}
+
+// Small state of one GMRES cycle, all on the device (column-major R of restart+1 rows).
+struct GmresState {
+    double* R;        // [(restart+1) * restart] rotated Hessenberg (upper triangular after rotation)
+    double* cs;       // [restart]
+    double* sn;       // [restart]
+    double* g;        // [restart+1] rotated right-hand side
+    double* hcol;     // [restart+1] current Hessenberg column (sum of the two Gram-Schmidt passes)
+    double* yv;       // [restart]   solution of R y = g
+    double* scal;     // [0] beta or h_{j+1,j}; [1] its reciprocal; [2] |g_{j+1}|; [3] ||b||
+};
+
+// Column j of the Hessenberg matrix: hcol[0..j] from Gram-Schmidt, h_{j+1,j} = sqrt(sum norm_partial);
+// earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").
+__global__ void hessenberg_kernel(GmresState st, int j, int ldr, const double* __restrict__ norm_partial, int nblk)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) s += norm_partial[b];
+    const double hn = sqrt(s);
+    st.scal[0] = hn;
+    st.scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
+    double* col = st.R + (size_t)j * ldr;
+    for (int i = 0; i <= j; ++i) col[i] = st.hcol[i];
+    col[j + 1] = hn;
+    for (int i = 0; i < j; ++i) {
+        const double t = st.cs[i] * col[i] + st.sn[i] * col[i + 1];
+        col[i + 1] = -st.sn[i] * col[i] + st.cs[i] * col[i + 1];
+        col[i] = t;
+    }
+    const double d = hypot(col[j], col[j + 1]);
+    const double c = d > 0.0 ? col[j] / d : 1.0, sgn = d > 0.0 ? col[j + 1] / d : 0.0;
+    st.cs[j] = c; st.sn[j] = sgn;
+    col[j] = d; col[j + 1] = 0.0;
+    st.g[j + 1] = -sgn * st.g[j];
+    st.g[j] = c * st.g[j];
+    st.scal[2] = fabs(st.g[j + 1]);
+}
+
+// beta = sqrt(sum partial) at the start of a cycle: g = (beta, 0, ...), scal[0..1] = beta, 1/beta;
+// with set_bnorm, scal[3] = beta (the first cycle starts from x0 = 0, so r0 = b).
+__global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int restart, int set_bnorm)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) s += norm_partial[b];
+    const double beta = sqrt(s);
+    st.scal[0] = beta; st.scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; st.scal[2] = beta;
+    if (set_bnorm) st.scal[3] = beta;
+    for (int i = 0; i <= restart; ++i) st.g[i] = i == 0 ? beta : 0.0;
+}
+
+// R y = g for the first k columns (back substitution).
+__global__ void solve_y_kernel(GmresState st, int k, int ldr)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    for (int i = k - 1; i >= 0; --i) {
+        double s = st.g[i];
+        for (int c = i + 1; c < k; ++c) s -= st.R[(size_t)c * ldr + i] * st.yv[c];
+        st.yv[i] = s / st.R[(size_t)i * ldr + i];
+    }
+}
+
+// out[i] = (*scale_ptr) * in[i]
+__global__ void scale_kernel(const double* __restrict__ in, const double* __restrict__ scale_ptr, double* __restrict__ out, int64_t n)
+{
+    const double s = *scale_ptr;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = s * in[i];
+}
+
+// out[i] = sum_{v<k} y[v] V[v][i]
+__global__ void combine_kernel(const double* __restrict__ V, int64_t ldv, int k, const double* __restrict__ y,
+                               double* __restrict__ out, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int v = 0; v < k; ++v) s += y[v] * V[(int64_t)v * ldv + i];
+        out[i] = s;
+    }
+}
+
+// y[i] = alpha * x[i] + beta * y[i]   (beta == 0 overwrites)
+__global__ void axpby_kernel(double alpha, const double* __restrict__ x, double beta, double* __restrict__ y, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        y[i] = beta == 0.0 ? alpha * x[i] : alpha * x[i] + beta * y[i];
+}
+
+// |w chunk|^2 per CTA (the norm of a vector through the same two-stage reduction)
+__global__ void __launch_bounds__(kVecThreads)
+norm_partial_kernel(const double* __restrict__ w, int64_t n, double* __restrict__ norm_partial)
+{
+    __shared__ double red[kVecThreads / 32];
+    int64_t lo, hi; chunk_of(n, lo, hi);
+    double nrm = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) nrm += w[i] * w[i];
+    nrm = warp_sum(nrm);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = nrm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int k = 0; k < kVecThreads / 32; ++k) s += red[k];
+        norm_partial[blockIdx.x] = s;
+    }
+}
+
+__global__ void to_float_kernel(const double* __restrict__ in, float* __restrict__ out, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = (float)in[i];
+}
+__global__ void to_double_kernel(const float* __restrict__ in, double* __restrict__ out, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = (double)in[i];
+}
+
+}  // namespace
+
+// =================================================================== host side
+namespace {
+
+thread_local int64_t* t_tables = nullptr;      // host staging of the offset tables (grown on demand)
+thread_local size_t t_tables_cap = 0;
+
+inline bool finite_pos(double v) { return v > 0.0 && isfinite(v); }
+inline unsigned warp_grid(int64_t n_bodies, int threads) { return (unsigned)((n_bodies * 32 + threads - 1) / threads); }
+
+#define RPY_CUDA_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return rpy::set_cuda_error(e__); } while (0)
+
+rpy_status check_bodies(int64_t n_blobs, int64_t n_bodies)
+{
+    if (n_blobs < 0 || n_blobs > RPY_MAX_BLOBS || n_bodies < 0 || n_bodies > n_blobs) return RPY_ERR_ARG;
+    return RPY_OK;
+}
+
+// Solver workspace, carved from one caller-owned buffer.
+struct SolveWs {
+    int64_t n; size_t vec_bytes;
+    double *V, *w, *z, *x, *b;
+    GmresState st; int ldr;
+    double *partial, *norm_partial;
+    float *pos32, *lam32, *vel32;
+    void* mv; size_t mv_bytes;
+    size_t total;
+};
+
+SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, void* base)
+{
+    SolveWs W;
+    unsigned char* p = static_cast<unsigned char*>(base);
+    size_t at = 0;
+    auto take = [&](size_t bytes) { unsigned char* r = p ? p + at : nullptr; at = align_up(at + bytes, kAlign); return r; };
+    W.n = 3 * n_blobs + 6 * n_bodies;
+    W.vec_bytes = align_up((size_t)W.n * 8, kAlign);
+    W.V = (double*)take(W.vec_bytes * (size_t)(restart + 1));
+    W.w = (double*)take(W.vec_bytes); W.z = (double*)take(W.vec_bytes);
+    W.x = (double*)take(W.vec_bytes); W.b = (double*)take(W.vec_bytes);
+    W.ldr = restart + 1;
+    W.st.R = (double*)take((size_t)(restart + 1) * restart * 8);
+    W.st.cs = (double*)take((size_t)restart * 8); W.st.sn = (double*)take((size_t)restart * 8);
+    W.st.g = (double*)take((size_t)(restart + 1) * 8); W.st.hcol = (double*)take((size_t)(restart + 1) * 8);
+    W.st.yv = (double*)take((size_t)restart * 8); W.st.scal = (double*)take(8 * 8);
+    W.partial = (double*)take((size_t)kVecBlocks * (restart + 1) * 8);
+    W.norm_partial = (double*)take((size_t)kVecBlocks * 8);
+    if (prec == RPY_PREC_F32_ACC64) {
+        W.pos32 = (float*)take((size_t)n_blobs * 12); W.lam32 = (float*)take((size_t)n_blobs * 12);
+        W.vel32 = (float*)take((size_t)n_blobs * 12);
+    } else { W.pos32 = W.lam32 = W.vel32 = nullptr; }
+    W.mv_bytes = rpy_matvec_workspace_bytes(prec, n_blobs, 1);
+    W.mv = take(W.mv_bytes);
+    W.total = at;
+    return W;
+}
+
+inline int64_t vec_stride(const SolveWs& W) { return (int64_t)(W.vec_bytes / 8); }
+
+// out = [M lambda - K U ; -K^T lambda], Eq. (11)'s operator.  pos32 must hold float(pos) for the fp32 product.
+rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* pos, const double* q,
+                  const int64_t* off, double a, double eta, const double* in, double* out, const SolveWs& W,
+                  cudaStream_t st)
+{
+    rpy_status s;
+    if (prec == RPY_PREC_F64) {
+        s = wall ? rpy_wall_matvec(prec, N, 1, pos, in, out, a, eta, W.mv, W.mv_bytes, st)
+                 : rpy_free_matvec(prec, N, 1, pos, in, out, a, eta, W.mv, W.mv_bytes, st);
+        if (s != RPY_OK) return s;
+    } else {
+        to_float_kernel<<<kVecBlocks, 256, 0, st>>>(in, W.lam32, 3 * N);
+        s = wall ? rpy_wall_matvec(prec, N, 1, W.pos32, W.lam32, W.vel32, a, eta, W.mv, W.mv_bytes, st)
+                 : rpy_free_matvec(prec, N, 1, W.pos32, W.lam32, W.vel32, a, eta, W.mv, W.mv_bytes, st);
+        if (s != RPY_OK) return s;
+        to_double_kernel<<<kVecBlocks, 256, 0, st>>>(W.vel32, out, 3 * N);
+    }
+    k_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(pos, q, off, in + 3 * N, -1.0, 1.0, out, nb);
+    kt_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(pos, q, off, in, -1.0, 0.0, out + 3 * N, nb);
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, cudaStream_t st)
+{
+    precond_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+rpy_status rpy_rigid_K_apply(int64_t n_blobs, int64_t n_bodies, const double* d_pos, const double* d_q,
+                             const int64_t* d_offsets, const double* d_U, double alpha, double beta,
+                             double* d_out, void* cuda_stream)
+{
+    rpy_status s = check_bodies(n_blobs, n_bodies);
+    if (s != RPY_OK) return s;
+    if (n_blobs == 0 || n_bodies == 0) return RPY_OK;
+    if (!d_pos || !d_q || !d_offsets || !d_U || !d_out) return RPY_ERR_NULL;
+    if (!isfinite(alpha) || !isfinite(beta)) return RPY_ERR_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    k_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_U, alpha, beta, d_out, n_bodies);
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double* d_pos, const double* d_q,
+                              const int64_t* d_offsets, const double* d_lambda, double alpha, double beta,
+                              double* d_out, void* cuda_stream)
+{
+    rpy_status s = check_bodies(n_blobs, n_bodies);
+    if (s != RPY_OK) return s;
+    if (n_blobs == 0 || n_bodies == 0) return RPY_OK;
+    if (!d_pos || !d_q || !d_offsets || !d_lambda || !d_out) return RPY_ERR_NULL;
+    if (!isfinite(alpha) || !isfinite(beta)) return RPY_ERR_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    kt_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_lambda, alpha, beta, d_out, n_bodies);
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+size_t rpy_rigid_precond_bytes(int64_t n_bodies, const int64_t* h_offsets)
+{
+    PrecondLayout L;
+    if (!layout_of(n_bodies, h_offsets, L) || L.n_blobs > RPY_MAX_BLOBS) return 0;
+    return L.total;
+}
+
+rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, const double* d_pos,
+                                   const double* d_q, const int64_t* h_offsets, double a, double eta,
+                                   void* d_precond, size_t precond_bytes, void* cuda_stream)
+{
+    rpy_status s = check_bodies(n_blobs, n_bodies);
+    if (s != RPY_OK) return s;
+    if (!finite_pos(a) || !finite_pos(eta)) return RPY_ERR_ARG;
+    if (n_bodies == 0) return n_blobs == 0 ? RPY_OK : RPY_ERR_ARG;
+    if (!d_pos || !d_q || !h_offsets || !d_precond) return RPY_ERR_NULL;
+    PrecondLayout L;
+    if (!layout_of(n_bodies, h_offsets, L) || L.n_blobs != n_blobs) return RPY_ERR_ARG;
+    if (precond_bytes < L.total || ((uintptr_t)d_precond % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // host tables: header, offsets, matrix offsets -> one staging array, copied before returning
+    const size_t words = 4 + 2 * (size_t)(n_bodies + 1);
+    if (t_tables_cap < words) {
+        int64_t* nt = static_cast<int64_t*>(realloc(t_tables, words * sizeof(int64_t)));
+        if (!nt) return RPY_ERR_ARG;
+        t_tables = nt; t_tables_cap = words;
+    }
+    int64_t* hdr = t_tables; int64_t* off = hdr + 4; int64_t* mo = off + (n_bodies + 1);
+    hdr[0] = kMagic; hdr[1] = n_bodies; hdr[2] = n_blobs; hdr[3] = L.total_mat;
+    int64_t acc = 0; size_t smem = 0;
+    for (int64_t p = 0; p <= n_bodies; ++p) {
+        off[p] = h_offsets[p]; mo[p] = acc;
+        if (p < n_bodies) {
+            const int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]);
+            acc += m * m;
+            if (m <= kSmemBodyM) { size_t need = ((size_t)(m | 1) * m + 6 * m) * 8; if (need > smem) smem = need; }
+        }
+    }
+    unsigned char* base = static_cast<unsigned char*>(d_precond);
+    RPY_CUDA_TRY(cudaMemcpyAsync(base, hdr, 4 * 8, cudaMemcpyHostToDevice, st));
+    RPY_CUDA_TRY(cudaMemcpyAsync(base + L.offsets_at, off, (size_t)(n_bodies + 1) * 8, cudaMemcpyHostToDevice, st));
+    RPY_CUDA_TRY(cudaMemcpyAsync(base + L.matoff_at, mo, (size_t)(n_bodies + 1) * 8, cudaMemcpyHostToDevice, st));
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));      // the staging array may be reused by the next call
+    PrecondView v = view_of(d_precond, n_bodies, n_blobs, L.total_mat);
+    const double PI = 3.14159265358979323846;
+    const double scale = 1.0 / (6.0 * PI * eta * a);
+    if (wall) {
+        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        precond_build_kernel<true><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                  v.factors, v.Y, v.Nt, 1.0 / a, scale);
+    } else {
+        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        precond_build_kernel<false><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                   v.factors, v.Y, v.Nt, 1.0 / a, scale);
+    }
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+__global__ void first_bad_kernel(const void* precond, int64_t n_bodies, long long* out)
+{
+    const int64_t* hdr = static_cast<const int64_t*>(precond);
+    if (hdr[0] != kMagic || hdr[1] != n_bodies) { if (blockIdx.x == 0 && threadIdx.x == 0) *out = -2; return; }
+    const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, hdr[2], hdr[3]);
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_bodies; p += (int64_t)gridDim.x * blockDim.x)
+        if (pv.info[p] != 0) atomicMin(out, (long long)p);
+}
+
+// Reads the first failed body through scratch[0] (a device int64 the caller owns).
+rpy_status first_bad(int64_t n_bodies, const void* precond, long long* d_scratch, int64_t* h_first, cudaStream_t st)
+{
+    const long long big = (long long)1 << 62;
+    RPY_CUDA_TRY(cudaMemcpyAsync(d_scratch, &big, 8, cudaMemcpyHostToDevice, st));
+    first_bad_kernel<<<64, 256, 0, st>>>(precond, n_bodies, d_scratch);
+    RPY_CUDA_TRY(cudaGetLastError());
+    long long r = 0;
+    RPY_CUDA_TRY(cudaMemcpyAsync(&r, d_scratch, 8, cudaMemcpyDeviceToHost, st));
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));
+    if (r == -2) { *h_first = -1; return RPY_ERR_ARG; }          // not a preconditioner of these bodies
+    *h_first = r == big ? -1 : (int64_t)r;
+    return r == big ? RPY_OK : st_of(RPY_ERR_NOT_SPD);
+}
+
+}  // namespace
+
+extern "C" {
+
+rpy_status rpy_rigid_precond_info(int64_t n_bodies, const void* d_precond, int64_t* h_first_bad_body, void* cuda_stream)
+{
+    if (n_bodies < 1) return RPY_ERR_ARG;
+    if (!d_precond || !h_first_bad_body) return RPY_ERR_NULL;
+    // header word [0] is the magic; words [1..3] are sizes: the unused tail of the 256-byte header is scratch
+    long long* scratch = reinterpret_cast<long long*>(const_cast<void*>(d_precond)) + 8;
+    return first_bad(n_bodies, d_precond, scratch, h_first_bad_body, static_cast<cudaStream_t>(cuda_stream));
+}
+
+rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void* d_precond,
+                                   const double* d_in, double* d_out, void* cuda_stream)
+{
+    rpy_status s = check_bodies(n_blobs, n_bodies);
+    if (s != RPY_OK) return s;
+    if (n_bodies == 0) return RPY_OK;
+    if (!d_precond || !d_in || !d_out) return RPY_ERR_NULL;
+    const size_t bytes = (size_t)(3 * n_blobs + 6 * n_bodies) * 8;
+    const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
+    if (a < b + bytes && b < a + bytes) return RPY_ERR_ALIAS;
+    return precond_apply(n_blobs, n_bodies, d_precond, d_in, d_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t* h_offsets, const void* d_precond, int64_t body,
+                                 double* d_factor, double* d_body_mobility, void* cuda_stream)
+{
+    if (!h_offsets || !d_precond) return RPY_ERR_NULL;
+    PrecondLayout L;
+    if (!layout_of(n_bodies, h_offsets, L) || body < 0 || body >= n_bodies) return RPY_ERR_ARG;
+    PrecondView v = view_of(const_cast<void*>(d_precond), n_bodies, L.n_blobs, L.total_mat);
+    int64_t mo = 0;
+    for (int64_t p = 0; p < body; ++p) { int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]); mo += m * m; }
+    const int64_t m = 3 * (h_offsets[body + 1] - h_offsets[body]);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (d_factor) RPY_CUDA_TRY(cudaMemcpyAsync(d_factor, v.factors + mo, (size_t)m * m * 8, cudaMemcpyDeviceToDevice, st));
+    if (d_body_mobility) RPY_CUDA_TRY(cudaMemcpyAsync(d_body_mobility, v.Nt + body * 36, 36 * 8, cudaMemcpyDeviceToDevice, st));
+    return RPY_OK;
+}
+
+size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart)
+{
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64) return 0;
+    if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1 || restart < 1 || restart > RPY_RIGID_MAX_RESTART) return 0;
+    return carve(matvec_prec, n_blobs, n_bodies, restart, nullptr).total;
+}
+
+rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
+                                  const double* d_pos, const double* d_q, const int64_t* d_offsets,
+                                  double a, double eta, const double* d_in, double* d_out,
+                                  void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    rpy_status s = check_bodies(n_blobs, n_bodies);
+    if (s != RPY_OK || n_bodies < 1) return RPY_ERR_ARG;
+    if (!finite_pos(a) || !finite_pos(eta)) return RPY_ERR_ARG;
+    if (!d_pos || !d_q || !d_offsets || !d_in || !d_out || !d_workspace) return RPY_ERR_NULL;
+    SolveWs W = carve(matvec_prec, n_blobs, n_bodies, 1, d_workspace);
+    if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (matvec_prec == RPY_PREC_F32_ACC64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * n_blobs);
+    return saddle(wall, matvec_prec, n_blobs, n_bodies, d_pos, d_q, d_offsets, a, eta, d_in, d_out, W, st);
+}
+
+rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
+                                    const double* d_pos, const double* d_q, const int64_t* d_offsets,
+                                    const double* d_F, const double* d_slip, double a, double eta,
+                                    const void* d_precond, double tol, int restart, int max_iter,
+                                    double* d_lambda, double* d_U,
+                                    double* h_history, int* h_n_iter, double* h_rel_resid,
+                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1) return RPY_ERR_ARG;
+    if (!finite_pos(a) || !finite_pos(eta) || !(tol >= 0.0) || restart < 1 || restart > RPY_RIGID_MAX_RESTART || max_iter < 1)
+        return RPY_ERR_ARG;
+    if (!d_pos || !d_q || !d_offsets || !d_F || !d_precond || !d_lambda || !d_U || !d_workspace) return RPY_ERR_NULL;
+    SolveWs W = carve(matvec_prec, n_blobs, n_bodies, restart, d_workspace);
+    if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t N = n_blobs, nb = n_bodies, n = W.n, ldv = vec_stride(W);
+
+    int64_t bad = -1;
+    rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
+    if (s != RPY_OK) return s;
+    if (matvec_prec == RPY_PREC_F32_ACC64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * N);
+
+    // b = [slip; -F], x = 0, r0 = b
+    if (d_slip) RPY_CUDA_TRY(cudaMemcpyAsync(W.b, d_slip, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
+    else RPY_CUDA_TRY(cudaMemsetAsync(W.b, 0, (size_t)N * 24, st));
+    axpby_kernel<<<64, 256, 0, st>>>(-1.0, d_F, 0.0, W.b + 3 * N, 6 * nb);
+    RPY_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, st));
+    norm_partial_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.b, n, W.norm_partial);
+    cycle_start_kernel<<<1, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, restart, 1);
+    double bnorm = 0.0;
+    RPY_CUDA_TRY(cudaMemcpyAsync(&bnorm, W.st.scal + 3, 8, cudaMemcpyDeviceToHost, st));
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));
+    if (h_history) h_history[0] = 1.0;
+    int n_iter = 0; double rel = 1.0;
+    if (!(bnorm > 0.0)) {
+        RPY_CUDA_TRY(cudaMemsetAsync(d_lambda, 0, (size_t)N * 24, st));
+        RPY_CUDA_TRY(cudaMemsetAsync(d_U, 0, (size_t)nb * 48, st));
+        RPY_CUDA_TRY(cudaStreamSynchronize(st));
+        if (h_n_iter) *h_n_iter = 0;
+        if (h_rel_resid) *h_rel_resid = 0.0;
+        return isfinite(bnorm) ? RPY_OK : RPY_ERR_ARG;
+    }
+    const double* r = W.b;
+    bool done = false;
+    while (!done) {
+        scale_kernel<<<kVecBlocks, 256, 0, st>>>(r, W.st.scal + 1, W.V, n);          // v_0 = r / beta
+        int k = 0;
+        for (int j = 0; j < restart; ++j) {
+            const double* vj = W.V + (int64_t)j * ldv;
+            if ((s = precond_apply(N, nb, d_precond, vj, W.z, st)) != RPY_OK) return s;
+            if ((s = saddle(wall, matvec_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, W, st)) != RPY_OK) return s;
+            ++n_iter;
+            // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
+            dots_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial);
+            update_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial, W.st.hcol, 0, W.norm_partial);
+            dots_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial);
+            update_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial, W.st.hcol, 1, W.norm_partial);
+            hessenberg_kernel<<<1, 32, 0, st>>>(W.st, j, W.ldr, W.norm_partial, kVecBlocks);
+            if (j + 1 <= restart) scale_kernel<<<kVecBlocks, 256, 0, st>>>(W.w, W.st.scal + 1, W.V + (int64_t)(j + 1) * ldv, n);
+            double res = 0.0;
+            RPY_CUDA_TRY(cudaMemcpyAsync(&res, W.st.scal + 2, 8, cudaMemcpyDeviceToHost, st));
+            RPY_CUDA_TRY(cudaStreamSynchronize(st));
+            rel = res / bnorm;
+            if (h_history) h_history[n_iter] = rel;
+            k = j + 1;
+            if (!(rel > tol) || n_iter >= max_iter) { done = true; break; }
+        }
+        // x += P^-1 (V_k y),  R y = g
+        solve_y_kernel<<<1, 32, 0, st>>>(W.st, k, W.ldr);
+        combine_kernel<<<kVecBlocks, 256, 0, st>>>(W.V, ldv, k, W.st.yv, W.w, n);
+        if ((s = precond_apply(N, nb, d_precond, W.w, W.z, st)) != RPY_OK) return s;
+        axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.z, 1.0, W.x, n);
+        if (done) break;
+        // restart: r = b - A x
+        if ((s = saddle(wall, matvec_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, W, st)) != RPY_OK) return s;
+        axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.b, -1.0, W.w, n);
+        norm_partial_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.w, n, W.norm_partial);
+        cycle_start_kernel<<<1, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, restart, 0);
+        r = W.w;
+    }
+    RPY_CUDA_TRY(cudaMemcpyAsync(d_lambda, W.x, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
+    RPY_CUDA_TRY(cudaMemcpyAsync(d_U, W.x + 3 * N, (size_t)nb * 48, cudaMemcpyDeviceToDevice, st));
+    RPY_CUDA_TRY(cudaGetLastError());
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));
+    if (h_n_iter) *h_n_iter = n_iter;
+    if (h_rel_resid) *h_rel_resid = rel;
+    return RPY_OK;
+}
+
+}  // extern "C"

@@ -217,3 +217,40 @@ def sample_rows(n: int, n_rows: int, seed: int = 12345) -> np.ndarray:
         return np.arange(n, dtype=np.int64)
     rng = np.random.default_rng(seed)
     return np.sort(rng.choice(n, size=n_rows, replace=False)).astype(np.int64)
+
+
+def cylinder_template(n_rings: int = 10, per_ring: int = 6, radius: float = 1.2, spacing: float = 2.0) -> np.ndarray:
+    """Blobs on the surface of a cylinder along x (rings of `per_ring` blobs, alternate rings turned by
+    half a step): the surface-resolved rod of PAPER.md:641, scaled down.  Centre of mass at the origin."""
+    pts = []
+    for r in range(n_rings):
+        x = (r - 0.5 * (n_rings - 1)) * spacing
+        for s in range(per_ring):
+            th = 2.0 * np.pi * (s + 0.5 * (r % 2)) / per_ring
+            pts.append((x, radius * np.cos(th), radius * np.sin(th)))
+    return np.array(pts)
+
+
+def mixed_suspension(seed: int = 0, n_groups: int = 2):
+    """Bodies of different sizes in one suspension (15-blob boomerangs, 42-blob shells of radius 3,
+    60-blob cylinders), `n_groups` of each, on a jittered lattice of spacing 40a, random orientations,
+    every blob at z >= 1.1a.  Returns (pos [N,3], Bodies, lambda [N,3]).  Exercises ragged offsets and
+    both the shared-memory (3*blobs <= 162) and the global-memory factorisation paths."""
+    rng = np.random.default_rng(seed)
+    templates = [boomerang_template(), 3.0 * shell_template(42), cylinder_template()]
+    pos, q, offsets = [], [], [0]
+    slot = 0
+    for g in range(n_groups):
+        for t in templates:
+            quat = rng.standard_normal(4)
+            R = quat_to_rot((quat / np.linalg.norm(quat))[None, :])[0]
+            c = np.array([40.0 * (slot % 4) + rng.uniform(-3, 3), 40.0 * (slot // 4) + rng.uniform(-3, 3), 0.0])
+            body = t @ R.T
+            c[2] = 1.1 - body[:, 2].min() + rng.uniform(0.2, 3.0)
+            body = body + c
+            pos.append(body); q.append(body.mean(axis=0)); offsets.append(offsets[-1] + body.shape[0])
+            slot += 1
+    pos = np.concatenate(pos, axis=0)
+    b = Bodies(np.array(offsets, dtype=np.int64), np.array(q), rng.standard_normal((len(q), 6)))
+    lam = rng.standard_normal(pos.shape)
+    return pos, b, lam

@@ -174,3 +174,50 @@ def test_product_never_imports_the_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1602_02170_b200 import" not in txt and "import paper_1602_02170_b200" not in txt
+
+
+# ------------------------------------------------------------------ include/rpy_rigid.h
+RIGID_HEADER = os.path.join(ROOT, "include", "rpy_rigid.h")
+
+
+def test_rigid_header_symbols_are_exported_and_bound():
+    from paper_1602_02170_b200 import rigid
+    src = re.sub(r"/\*.*?\*/", "", open(RIGID_HEADER).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(rpy_rigid_[a-z0-9_A-Z]+)\s*\(", src)))
+    lib = rigid._lib()
+    assert len(names) == 10
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in rpy_rigid.h but not exported"
+    assert set(names) == set(rigid.SIGNATURES)
+
+
+def test_rigid_host_arithmetic_and_argument_checks():
+    import numpy as np
+    from paper_1602_02170_b200 import rigid
+    lib = rigid._lib()
+    pb = rigid.rpy_rigid_precond_bytes
+    assert pb([0, 15, 30]) > 2 * 45 * 45 * 8 and pb([0, 15, 30]) % 256 == 0
+    assert pb([0, 15, 57, 117]) > pb([0, 15, 57])
+    assert pb([1, 15]) == 0 and pb([0, 5, 5]) == 0 and pb([0, 600]) == 0     # bad start, empty body, body too large
+    w = rigid.rpy_rigid_solve_workspace_bytes
+    n, nb = 15000, 1000
+    assert w("f64", n, nb, 60) >= 65 * (3 * n + 6 * nb) * 8
+    assert w("f32", n, nb, 60) > 0 and w("f64", n, nb, 0) == 0 and w("f64", n, nb, 129) == 0 and w("f64", n, 0, 10) == 0
+    assert w("f64", n, nb, 30) < w("f64", n, nb, 60)
+    # argument errors are detected before any CUDA call (works without a GPU)
+    one = ctypes.c_void_p(256)
+    assert lib.rpy_rigid_K_apply(10, 2, None, one, one, one, 1.0, 0.0, one, None) == 1
+    assert lib.rpy_rigid_K_apply(-1, 2, one, one, one, one, 1.0, 0.0, one, None) == 2
+    assert lib.rpy_rigid_KT_apply(10, 11, one, one, one, one, 1.0, 0.0, one, None) == 2
+    assert lib.rpy_rigid_KT_apply(10, 2, one, one, one, one, float("nan"), 0.0, one, None) == 2
+    off = (ctypes.c_int64 * 3)(0, 4, 10)
+    assert lib.rpy_rigid_precond_build(1, 10, 2, one, one, off, -1.0, 1.0, one, 1 << 20, None) == 2
+    assert lib.rpy_rigid_precond_build(1, 11, 2, one, one, off, 1.0, 1.0, one, 1 << 20, None) == 2
+    assert lib.rpy_rigid_precond_build(1, 10, 2, one, one, off, 1.0, 1.0, one, 16, None) == 4
+    assert lib.rpy_rigid_precond_apply(10, 2, one, one, one, None) == 3            # in aliases out
+    n_it, rr = ctypes.c_int(), ctypes.c_double()
+    args = lambda tol, restart, ws: (1, 0, 10, 2, one, one, one, one, None, 1.0, 1.0, one, tol, restart, 50, one, one,
+                                     None, ctypes.byref(n_it), ctypes.byref(rr), one, ws, None)
+    assert lib.rpy_rigid_mobility_solve(*args(-1.0, 10, 1 << 30)) == 2
+    assert lib.rpy_rigid_mobility_solve(*args(1e-8, 500, 1 << 30)) == 2
+    assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, 64)) == 4
