@@ -283,6 +283,50 @@ def time_e2e(torch, binding, wl, prec, variant, steps, warmup):
             "d2h_bytes_per_step": int(out.numel() * es), "ms_per_step": t * 1e3, "checksum_abs_u": checksum}
 
 
+def time_solve(torch, cfg: int, matvec_prec: str, tol: float, restart: int = 60):
+    """The rigid-multiblob mobility solve (SURVEY 8(f) N1+N2) on a rigid-body workload: preconditioner
+    build, GMRES on Eq. (11) to `tol`, and the per-application cost of its pieces (CUDA events)."""
+    from paper_1602_02170_b200 import rigid, workloads
+    wl = workloads.make(cfg, k=1) if cfg != 5 else workloads.make(3)
+    hb = workloads.bodies_of(wl)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=np.float64)).to(dev)
+    b = rigid.bodies(t(wl.pos), t(hb.q), hb.offsets)
+    F = t(hb.F)
+    slip = t(0.1 * np.random.default_rng(8).standard_normal(wl.pos.shape))
+
+    def timed(fn, reps=3):
+        fn(); torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            out = fn()
+        e1.record(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps, out
+
+    build_ms, pc = timed(lambda: rigid.rpy_rigid_precond_build(b, "wall", wl.a, wl.eta, check=False), reps=2)
+    rigid.rpy_rigid_precond_info(pc)
+    vec = torch.randn(b.n, dtype=torch.float64, device=dev)
+    out = torch.empty_like(vec)
+    apply_ms, _ = timed(lambda: rigid.rpy_rigid_precond_apply(pc, vec, out=out), reps=10)
+    saddle_ms, _ = timed(lambda: rigid.rpy_rigid_saddle_apply(b, vec, "wall", wl.a, wl.eta, matvec_prec), reps=3)
+    ws = torch.empty(rigid.rpy_rigid_solve_workspace_bytes(matvec_prec, b.n_blobs, b.n_bodies, restart),
+                     dtype=torch.uint8, device=dev)
+    solve = lambda: rigid.rpy_rigid_mobility_solve(b, pc, F, slip, "wall", wl.a, wl.eta, tol=tol, restart=restart,
+                                                   matvec_prec=matvec_prec, workspace=ws)
+    solve(); torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = solve()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    it = max(1, r["n_iter"])
+    return {"workload": wl.name, "n_blobs": b.n_blobs, "n_bodies": b.n_bodies, "matvec_prec": matvec_prec,
+            "tol": tol, "restart": restart, "n_iter": r["n_iter"], "rel_resid": r["rel_resid"],
+            "solve_ms": wall_ms, "ms_per_iter": wall_ms / it, "precond_build_ms": build_ms,
+            "precond_apply_ms": apply_ms, "saddle_apply_ms": saddle_ms,
+            "krylov_ms_per_iter": wall_ms / it - apply_ms - saddle_ms,
+            "matvec_share": saddle_ms / (wall_ms / it)}
+
+
 def run_ours(args):
     import torch
     from paper_1602_02170_b200 import binding, workloads
@@ -388,6 +432,15 @@ def run_ours(args):
                 log(f"[bench] extra {extra[-1]}")
                 del r2
             line["other_configs"] = extra
+            # --- next rows of SURVEY 8(f): the preconditioned GMRES mobility solve around the matvec
+            solves = []
+            for cfg, p, tol in ((2, "f64", 1e-8), (3, "f64", 1e-8), (3, "f32", 1e-5)):
+                try:
+                    solves.append(time_solve(torch, cfg, p, tol))
+                    log(f"[bench] solve {solves[-1]}")
+                except Exception as e:  # pragma: no cover
+                    solves.append({"config": cfg, "matvec_prec": p, "error": repr(e)})
+            line["rigid_solve"] = solves
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
