@@ -107,6 +107,36 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
                                 double a, double eta,
                                 void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* Rectangular product: velocities at n_targets points that are not the sources,
+ *   u_t = sum_{j < n_sources} M(r_t, r_j) lambda_j,
+ * the flow-field evaluation of Appendix B: "the velocity that a freely-moving
+ * tracer blob of a given size a' would have ... v(r) = sum_j M'(r - r_j) lambda'_j, where M' is the
+ * blob-blob mobility for blobs of radius a'".  Targets and sources share the radius `a` (= a' in
+ * the paper's use); a target that coincides with a source sees that source's self block.
+ *   d_target_pos [n_targets][3], d_source_pos [n_sources][3], d_force [n_rhs][n_sources][3],
+ *   d_vel [n_rhs][n_targets][3] (overwritten; all zero when n_sources == 0)
+ *   d_workspace: >= rpy_matvec_rect_workspace_bytes(), 256-byte aligned.
+ * Always the plain (bit-reproducible) all-pairs kernel.                                          */
+size_t rpy_matvec_rect_workspace_bytes(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs);
+rpy_status rpy_wall_matvec_rect(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs,
+                                const void *d_target_pos, const void *d_source_pos, const void *d_force,
+                                void *d_vel, double a, double eta,
+                                void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+rpy_status rpy_free_matvec_rect(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs,
+                                const void *d_target_pos, const void *d_source_pos, const void *d_force,
+                                void *d_vel, double a, double eta,
+                                void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Appendix B's source refinement: every blob i is replaced by n_sub small blobs at
+ * r_i + template[s] (the template, in real lengths, is the caller's choice: the paper does not say
+ * how the small blobs are placed) and its force is divided uniformly, lambda'_{i,s} = lambda_i / n_sub.
+ *   d_pos [n_blobs][3], d_force [n_rhs][n_blobs][3], d_template [n_sub][3]  ->
+ *   d_sub_pos [n_blobs * n_sub][3], d_sub_force [n_rhs][n_blobs * n_sub][3]   (sub-blob s of blob i at
+ *   index i * n_sub + s).  1 <= n_sub <= 4096; n_blobs * n_sub <= RPY_MAX_BLOBS.                  */
+rpy_status rpy_flow_subdivide(rpy_prec prec, int64_t n_blobs, int n_rhs, int n_sub,
+                              const void *d_pos, const void *d_force, const void *d_template,
+                              void *d_sub_pos, void *d_sub_force, void *cuda_stream);
+
 /* Host-buffer forms ("only the positions of the blobs need to be communicated",
  * here positions and forces go up, velocities come back).
  *   h_pos, h_force, h_vel : HOST pointers, layouts as above

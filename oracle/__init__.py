@@ -56,6 +56,9 @@ def _load():
         lib.rpy_oracle_matvec.argtypes = [ctypes.c_int, ctypes.c_int64, ctypes.c_int, dp, dp,
                                           ctypes.c_double, ctypes.c_double, ctypes.c_int64, ip, dp]
         lib.rpy_oracle_matvec.restype = None
+        lib.rpy_oracle_flow.argtypes = [ctypes.c_int, ctypes.c_int64, dp, ctypes.c_int64, dp, ctypes.c_int, dp,
+                                        ctypes.c_double, ctypes.c_double, dp]
+        lib.rpy_oracle_flow.restype = None
         lib.rpy_oracle_num_threads.argtypes = []
         lib.rpy_oracle_num_threads.restype = ctypes.c_int
         _lib = lib
@@ -122,6 +125,32 @@ def matvec(variant: int, pos, force, a: float = 1.0, eta: float = 1.0, rows=None
         _load().rpy_oracle_matvec(int(variant), n, k, _dptr(pos), _dptr(f3), float(a), float(eta),
                                   nrows, rptr, _dptr(out))
     return out[0] if single else out
+
+
+def flow(variant: int, targets, pos, force, a: float = 1.0, eta: float = 1.0) -> np.ndarray:
+    """Flow field of Appendix B: v(r_t) = sum_j M'(r_t, r_j) lambda_j, tracer radius a.
+
+    targets [nt,3]; pos [ns,3]; force [ns,3] or [k,ns,3].  Returns [nt,3] or [k,nt,3]."""
+    targets = _f64(targets); pos = _f64(pos); force = _f64(force)
+    nt, ns = targets.shape[0], pos.shape[0]
+    assert targets.shape == (nt, 3) and pos.shape == (ns, 3)
+    single = force.ndim == 2
+    k = 1 if single else force.shape[0]
+    f3 = np.ascontiguousarray(force.reshape(k, ns, 3))
+    out = np.zeros((k, nt, 3))
+    if nt > 0 and ns > 0:
+        _load().rpy_oracle_flow(int(variant), nt, _dptr(targets), ns, _dptr(pos), k, _dptr(f3), float(a), float(eta),
+                                _dptr(out))
+    return out[0] if single else out
+
+
+def subdivide(pos, force, template):
+    """Appendix B: blob i -> small blobs at r_i + template[s], lambda' = lambda_i / n_sub."""
+    pos = _f64(pos); force = _f64(force); template = _f64(template)
+    ns = template.shape[0]
+    sub_pos = (pos[:, None, :] + template[None, :, :]).reshape(-1, 3)
+    sub_force = np.repeat(force, ns, axis=-2) / ns
+    return sub_pos, sub_force
 
 
 def num_threads() -> int:

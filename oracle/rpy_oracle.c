@@ -176,6 +176,35 @@ void rpy_oracle_matvec(int variant, int64_t n, int k, const double *pos, const d
     }
 }
 
+/* Flow field, Appendix B: v(r_t) = sum_j M'(r_t, r_j) lambda'_j at targets that
+ * are not the sources; M' is the same pair tensor with the tracer radius as `a` (both blobs of the
+ * pair have that radius).  tgt [nt][3], src [ns][3], force [k][ns][3], vel [k][nt][3]. */
+void rpy_oracle_flow(int variant, int64_t nt, const double *tgt, int64_t ns, const double *src, int k,
+                     const double *force, double a, double eta, double *vel)
+{
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 4)
+#endif
+    for (int64_t t = 0; t < nt; ++t) {
+        long double acc[3 * k];
+        for (int q = 0; q < 3 * k; ++q) acc[q] = 0.0L;
+        for (int64_t j = 0; j < ns; ++j) {
+            double B[9];
+            rpy_oracle_pair(variant, tgt + 3 * t, src + 3 * j, a, eta, B);
+            for (int s = 0; s < k; ++s) {
+                const double *lam = force + ((size_t)s * ns + j) * 3;
+                for (int p = 0; p < 3; ++p)
+                    acc[3 * s + p] += (long double)B[3 * p + 0] * lam[0]
+                                    + (long double)B[3 * p + 1] * lam[1]
+                                    + (long double)B[3 * p + 2] * lam[2];
+            }
+        }
+        for (int s = 0; s < k; ++s)
+            for (int p = 0; p < 3; ++p)
+                vel[((size_t)s * nt + t) * 3 + p] = (double)acc[3 * s + p];
+    }
+}
+
 /* Threads the row loop actually uses (reported beside the timed baseline). */
 int rpy_oracle_num_threads(void)
 {

@@ -46,6 +46,10 @@ SIGNATURES = {
     "rpy_free_matvec": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_wall_matvec_rows": (_int, [_int, _i64, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_free_matvec_rows": (_int, [_int, _i64, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
+    "rpy_matvec_rect_workspace_bytes": (_sz, [_int, _i64, _i64, _int]),
+    "rpy_wall_matvec_rect": (_int, [_int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
+    "rpy_free_matvec_rect": (_int, [_int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
+    "rpy_flow_subdivide": (_int, [_int, _i64, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
     "rpy_matvec_host_scratch_bytes": (_sz, [_int, _i64, _int]),
     "rpy_wall_matvec_host": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_free_matvec_host": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
@@ -214,6 +218,67 @@ def rpy_free_matvec(pos: torch.Tensor, force: torch.Tensor, a: float = 1.0, eta:
                     rows: Optional[tuple] = None) -> torch.Tensor:
     """u = M lambda with the free-space RPY tensor, Eq. (9)."""
     return _matvec("rpy_free_matvec", pos, force, a, eta, out, workspace, rows)
+
+
+def rpy_matvec_rect_workspace_bytes(prec, n_targets: int, n_sources: int, n_rhs: int = 1) -> int:
+    return int(load_library().rpy_matvec_rect_workspace_bytes(_prec_code(prec), int(n_targets), int(n_sources), int(n_rhs)))
+
+
+def _matvec_rect(fn_name: str, targets, pos, force, a, eta, out, workspace):
+    lib = load_library()
+    _require_cuda(pos, "pos")
+    _require_cuda(force, "force")
+    _require_cuda(targets, "targets")
+    n, k, single = _shape_inputs(pos, force)
+    if targets.dim() != 2 or targets.shape[1] != 3 or targets.dtype != pos.dtype or not targets.is_contiguous():
+        raise ValueError("targets must be a contiguous [n_targets, 3] tensor of the positions' dtype")
+    nt = targets.shape[0]
+    prec = _prec_of(pos.dtype)
+    oshape = (nt, 3) if single else (k, nt, 3)
+    if out is None:
+        out = torch.empty(oshape, dtype=pos.dtype, device=pos.device)
+    elif tuple(out.shape) != oshape or out.dtype != pos.dtype or out.device != pos.device or not out.is_contiguous():
+        raise ValueError(f"out must be a contiguous {pos.dtype} tensor of shape {oshape} on {pos.device}")
+    need = rpy_matvec_rect_workspace_bytes(prec, nt, n, k)
+    if workspace is None:
+        workspace = torch.empty(max(need, 1), dtype=torch.uint8, device=pos.device)
+    with torch.cuda.device(pos.device):
+        stream = torch.cuda.current_stream(pos.device).cuda_stream
+        _check(getattr(lib, fn_name)(prec, nt, n, k, targets.data_ptr() or None, pos.data_ptr() or None,
+                                     force.data_ptr() or None, out.data_ptr() or None, float(a), float(eta),
+                                     workspace.data_ptr(), int(workspace.numel()), stream))
+    return out
+
+
+def rpy_wall_matvec_rect(targets: torch.Tensor, pos: torch.Tensor, force: torch.Tensor, a: float = 1.0,
+                         eta: float = 1.0, *, out=None, workspace=None) -> torch.Tensor:
+    """Velocities at `targets` [n_targets,3] induced by forces on the blobs at `pos` (wall tensor):
+    the flow-field evaluation of Appendix B with tracer radius a."""
+    return _matvec_rect("rpy_wall_matvec_rect", targets, pos, force, a, eta, out, workspace)
+
+
+def rpy_free_matvec_rect(targets: torch.Tensor, pos: torch.Tensor, force: torch.Tensor, a: float = 1.0,
+                         eta: float = 1.0, *, out=None, workspace=None) -> torch.Tensor:
+    return _matvec_rect("rpy_free_matvec_rect", targets, pos, force, a, eta, out, workspace)
+
+
+def rpy_flow_subdivide(pos: torch.Tensor, force: torch.Tensor, template: torch.Tensor):
+    """Appendix B's refinement: every blob -> len(template) small blobs at r_i + template[s], force
+    divided uniformly.  Returns (sub_pos [n*n_sub,3], sub_force shaped like force with n*n_sub blobs)."""
+    lib = load_library()
+    _require_cuda(pos, "pos")
+    n, k, single = _shape_inputs(pos, force)
+    if template.dim() != 2 or template.shape[1] != 3 or template.dtype != pos.dtype or not template.is_cuda \
+            or not template.is_contiguous():
+        raise ValueError("template must be a contiguous CUDA [n_sub, 3] tensor of the positions' dtype")
+    ns = template.shape[0]
+    sub_pos = torch.empty((n * ns, 3), dtype=pos.dtype, device=pos.device)
+    sub_force = torch.empty((n * ns, 3) if single else (k, n * ns, 3), dtype=pos.dtype, device=pos.device)
+    with torch.cuda.device(pos.device):
+        stream = torch.cuda.current_stream(pos.device).cuda_stream
+        _check(lib.rpy_flow_subdivide(_prec_of(pos.dtype), n, k, ns, pos.data_ptr() or None, force.data_ptr() or None,
+                                      template.data_ptr(), sub_pos.data_ptr() or None, sub_force.data_ptr() or None, stream))
+    return sub_pos, sub_force
 
 
 def rpy_matvec_phases(variant: str, pos: torch.Tensor, force: torch.Tensor, a: float = 1.0, eta: float = 1.0, *,

@@ -63,6 +63,24 @@ __global__ void prepack_kernel(const typename L::S* __restrict__ pos,
     }
 }
 
+// Targets that are not sources (rectangular product, "Computing flow fields"):
+// only the scaled coordinates are written, in the same record layout, so the all-pairs kernel
+// reads its targets the same way in both cases.  Rows beyond n_targets are never read.
+template <class L, int K>
+__global__ void prepack_targets_kernel(const typename L::S* __restrict__ pos, typename L::S* __restrict__ rec,
+                                       int64_t n_targets, double inv_a)
+{
+    using S = typename L::S;
+    using R = RecLayout<L, K>;
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_targets) return;
+    S* r = rec + (j / R::W) * R::LEN;
+    int l = (int)(j % R::W);
+    r[0 * R::W + l] = (S)((double)pos[3 * j + 0] * inv_a);
+    r[1 * R::W + l] = (S)((double)pos[3 * j + 1] * inv_a);
+    r[2 * R::W + l] = (S)((double)pos[3 * j + 2] * inv_a);
+}
+
 // ---------------------------------------------------------------------------- mbarrier / bulk copy
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -100,10 +118,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
 //   - float forms: per-target partial sums in V over FLUSH_G records (<= 128 sources), then
 //     adds them into double running sums (the "fp64 accumulation" of north_star);
 //   - double form: the running sums directly.
+// Targets are read from `trec` (same record layout; equal to `rec` for the square product).
 // Output: partial[chunk][s][row][3] in double (row relative to row_begin).
 template <class L, int K, bool WALL, int T, int BLOCK, int TILE_G, int FLUSH_G, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
-allpairs_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial,
+allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __restrict__ trec,
+                double* __restrict__ partial,
                 int64_t row_begin, int64_t row_count, int64_t n_tiles, int tiles_per_chunk)
 {
     using V = typename L::V;
@@ -145,7 +165,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, double* __restrict__ part
     for (int t = 0; t < T; ++t) {
         row[t] = (int64_t)blockIdx.x * (BLOCK * T) + t * BLOCK + tid;
         int64_t i = row_begin + (row[t] < row_count ? row[t] : row_count - 1);
-        const S* r = rec + (i / W) * R::LEN + (i % W);
+        const S* r = trec + (i / W) * R::LEN + (i % W);      // trec == rec unless targets differ from sources
         xi[t] = L::bc((double)r[0 * W]);
         yi[t] = L::bc((double)r[1 * W]);
         zi[t] = L::bc((double)r[2 * W]);
@@ -450,6 +470,25 @@ __global__ void finalise_kernel(const double* __restrict__ partial, S* __restric
     for (int c = 0; c < n_chunks; ++c) sum += partial[(int64_t)c * per_chunk + e];
     int64_t s = e / row_count3, q = e % row_count3;
     vel[s * vel_rhs_stride + q] = (S)(sum * scale);
+}
+
+// Appendix B: blob i -> n_sub small blobs at r_i + template[s], force lambda_i / n_sub.
+template <class S>
+__global__ void subdivide_kernel(const S* __restrict__ pos, const S* __restrict__ force, const S* __restrict__ tmpl,
+                                 S* __restrict__ sub_pos, S* __restrict__ sub_force, int64_t n_blobs, int n_rhs, int n_sub)
+{
+    const int64_t total = n_blobs * n_sub;
+    const S div = (S)n_sub;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = e / n_sub;
+        const int s = (int)(e % n_sub);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sub_pos[3 * e + c] = pos[3 * i + c] + tmpl[3 * s + c];
+        for (int r = 0; r < n_rhs; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                sub_force[((int64_t)r * total + e) * 3 + c] = force[((int64_t)r * n_blobs + i) * 3 + c] / div;
+    }
 }
 
 template <class S>

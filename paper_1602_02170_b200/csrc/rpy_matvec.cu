@@ -20,7 +20,7 @@ namespace {
 
 thread_local int g_last_cuda_error = 0;
 
-constexpr int kAbiVersion = 2;
+constexpr int kAbiVersion = 3;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
 constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
 constexpr int kMaxChunks = 64;
@@ -119,12 +119,14 @@ size_t records_bytes(rpy_prec prec, int64_t n, int K)
 
 // n_chunks * rows <= kTargetCtas * kBlock * kMaxT + rows  (n_chunks <= kTargetCtas / n_target_tiles + 1)
 // and n_chunks <= n_tiles, rows <= n.
-size_t partial_bytes_bound(rpy_prec prec, int64_t n, int K)
+// `rows` target rows against `n` sources (rows <= n for the square product; any ratio for the
+// rectangular one).
+size_t partial_bytes_bound(rpy_prec prec, int64_t n, int K, int64_t rows)
 {
     int ts = tile_sources_of(prec);
     int64_t n_tiles = (n + ts - 1) / ts;
-    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + 2 * n;   // symmetric path: chunks + 1 slices
-    int64_t b = n_tiles * n;
+    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + 2 * rows;   // symmetric path: chunks + 1 slices
+    int64_t b = n_tiles * rows;
     return align_up((size_t)(a < b ? a : b) * (size_t)K * 3 * sizeof(double), kAlign);
 }
 
@@ -132,7 +134,16 @@ size_t workspace_bytes(rpy_prec prec, int64_t n, int n_rhs)
 {
     if (n <= 0 || n_rhs < 1) return 0;
     int K = group_k(n_rhs);
-    return records_bytes(prec, n, K) + partial_bytes_bound(prec, n, K);
+    return records_bytes(prec, n, K) + partial_bytes_bound(prec, n, K, n);
+}
+
+// rectangular product: source records, target records, partials
+size_t rect_workspace_bytes(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs)
+{
+    if (n_targets <= 0 || n_sources <= 0 || n_rhs < 1) return 0;
+    int K = group_k(n_rhs);
+    return records_bytes(prec, n_sources, K) + records_bytes(prec, n_targets, K) +
+           partial_bytes_bound(prec, n_sources, K, n_targets);
 }
 
 inline rpy_status cuda_fail(cudaError_t e)
@@ -156,11 +167,11 @@ auto allpairs_fn()
 template <class L, int K> constexpr size_t allpairs_smem() { return 2 * (size_t)Shape<L, K>::TILE_G * rpy::RecLayout<L, K>::BYTES; }
 
 template <class L, int K, bool WALL, int T>
-cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, double* partial,
+cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typename L::S* trec, double* partial,
                             int64_t row_begin, int64_t rows, cudaStream_t st)
 {
     dim3 grid((unsigned)p.n_target_tiles, (unsigned)p.n_chunks);
-    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
+    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, trec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
     return cudaGetLastError();
 }
 
@@ -205,13 +216,25 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
 template <class L, int K>
 cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, typename L::S* vel,
-                      double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev)
+                      double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev,
+                      const typename L::S* tpos /* targets of the rectangular product, else nullptr */)
 {
     using S = typename L::S;
     S* rec = reinterpret_cast<S*>(ws);
     rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
-    double* partial = reinterpret_cast<double*>(ws + records_bytes(prec, n, K));
-    const bool sym = use_symmetric(n, K, row_begin, rows);
+    size_t at = records_bytes(prec, n, K);
+    const S* trec = rec;
+    if (tpos) {                                    // rows = n_targets, row_begin = 0
+        S* tr = reinterpret_cast<S*>(ws + at);
+        at += records_bytes(prec, rows, K);
+        int threads = 256;
+        rpy::prepack_targets_kernel<L, K><<<(unsigned)((rows + threads - 1) / threads), threads, 0, st>>>(tpos, tr, rows, 1.0 / a);
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return e0;
+        trec = tr;
+    }
+    double* partial = reinterpret_cast<double*>(ws + at);
+    const bool sym = !tpos && use_symmetric(n, K, row_begin, rows);
     const Plan p = make_plan(prec, n, K, rows);
     const SymPlan sp = make_sym_plan(n);
     const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
@@ -236,10 +259,10 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     } else {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
         constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
-        if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, partial, row_begin, rows, st)
-                               : launch_allpairs<L, K, true, 1>(p, rec, partial, row_begin, rows, st);
-        else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, partial, row_begin, rows, st)
-                               : launch_allpairs<L, K, false, 1>(p, rec, partial, row_begin, rows, st);
+        if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, trec, partial, row_begin, rows, st)
+                               : launch_allpairs<L, K, true, 1>(p, rec, trec, partial, row_begin, rows, st);
+        else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, trec, partial, row_begin, rows, st)
+                               : launch_allpairs<L, K, false, 1>(p, rec, trec, partial, row_begin, rows, st);
     }
     if (e != cudaSuccess) return e;
     if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[2]), st)) != cudaSuccess) return e;
@@ -259,12 +282,14 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
 template <class L>
 cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
                            const void* d_pos, const void* d_force, void* d_vel,
-                           double a, double eta, void* ws, cudaStream_t st, void* const* ev)
+                           double a, double eta, void* ws, cudaStream_t st, void* const* ev,
+                           const void* d_tpos = nullptr)
 {
     using S = typename L::S;
     cudaError_t ee;
     if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[0]), st)) != cudaSuccess) return ee;
     const S* pos = static_cast<const S*>(d_pos);
+    const S* tp = static_cast<const S*>(d_tpos);
     int done = 0;
     while (done < n_rhs) {
         int K = group_k(n_rhs - done);
@@ -273,10 +298,10 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
         unsigned char* w = static_cast<unsigned char*>(ws);
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
-            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
@@ -306,6 +331,37 @@ rpy_status matvec_rows(bool wall, rpy_prec prec, int64_t n, int n_rhs, int64_t r
     cudaError_t e = prec == RPY_PREC_F64
         ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev)
         : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
+
+// u_t = sum_j M(r_t, r_j) lambda_j for targets that are not the sources.
+rpy_status matvec_rect(bool wall, rpy_prec prec, int64_t nt, int64_t ns, int n_rhs, const void* d_tpos,
+                       const void* d_spos, const void* d_force, void* d_vel, double a, double eta,
+                       void* ws, size_t ws_bytes, void* stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (nt < 0 || ns < 0 || nt > RPY_MAX_BLOBS || ns > RPY_MAX_BLOBS || n_rhs < 1) return RPY_ERR_ARG;
+    if (!(a > 0.0) || !(eta > 0.0) || !isfinite(a) || !isfinite(eta)) return RPY_ERR_ARG;
+    if (nt == 0) return RPY_OK;
+    if (!d_vel) return RPY_ERR_NULL;
+    size_t es = elem_size(prec);
+    size_t vel_b = (size_t)nt * 3 * es * (size_t)n_rhs;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (ns == 0) {                                  // empty sum
+        cudaError_t e = cudaMemsetAsync(d_vel, 0, vel_b, st);
+        return e == cudaSuccess ? RPY_OK : cuda_fail(e);
+    }
+    if (!d_tpos || !d_spos || !d_force || !ws) return RPY_ERR_NULL;
+    size_t need = rect_workspace_bytes(prec, nt, ns, n_rhs);
+    if (ws_bytes < need || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    size_t spos_b = (size_t)ns * 3 * es;
+    if (overlaps(d_vel, vel_b, d_tpos, (size_t)nt * 3 * es) || overlaps(d_vel, vel_b, d_spos, spos_b) ||
+        overlaps(d_vel, vel_b, d_force, spos_b * (size_t)n_rhs) || overlaps(d_vel, vel_b, ws, need))
+        return RPY_ERR_ALIAS;
+    cudaError_t e = prec == RPY_PREC_F64
+        ? run_all_groups<rpy::Lane<double>>(wall, ns, n_rhs, 0, nt, d_spos, d_force, d_vel, a, eta, ws, st, nullptr, d_tpos)
+        : run_all_groups<rpy::Lane<float2>>(wall, ns, n_rhs, 0, nt, d_spos, d_force, d_vel, a, eta, ws, st, nullptr, d_tpos);
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
 }
@@ -399,6 +455,53 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs, int64
     if (n_blobs < 0) return RPY_ERR_ARG;
     return matvec_rows(false, prec, n_blobs, n_rhs, row_begin, row_count, d_pos, d_force, d_vel, a, eta,
                        d_workspace, workspace_bytes_, cuda_stream);
+}
+
+size_t rpy_matvec_rect_workspace_bytes(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return 0;
+    if (n_targets > RPY_MAX_BLOBS || n_sources > RPY_MAX_BLOBS) return 0;
+    return rect_workspace_bytes(prec, n_targets, n_sources, n_rhs);
+}
+
+rpy_status rpy_wall_matvec_rect(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs,
+                                const void* d_target_pos, const void* d_source_pos, const void* d_force,
+                                void* d_vel, double a, double eta, void* d_workspace, size_t workspace_bytes_,
+                                void* cuda_stream)
+{
+    return matvec_rect(true, prec, n_targets, n_sources, n_rhs, d_target_pos, d_source_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_free_matvec_rect(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs,
+                                const void* d_target_pos, const void* d_source_pos, const void* d_force,
+                                void* d_vel, double a, double eta, void* d_workspace, size_t workspace_bytes_,
+                                void* cuda_stream)
+{
+    return matvec_rect(false, prec, n_targets, n_sources, n_rhs, d_target_pos, d_source_pos, d_force, d_vel, a, eta,
+                       d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_flow_subdivide(rpy_prec prec, int64_t n_blobs, int n_rhs, int n_sub, const void* d_pos,
+                              const void* d_force, const void* d_template, void* d_sub_pos, void* d_sub_force,
+                              void* cuda_stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n_blobs < 0 || n_rhs < 1 || n_sub < 1 || n_sub > 4096 || n_blobs * (int64_t)n_sub > RPY_MAX_BLOBS) return RPY_ERR_ARG;
+    if (n_blobs == 0) return RPY_OK;
+    if (!d_pos || !d_force || !d_template || !d_sub_pos || !d_sub_force) return RPY_ERR_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t total = n_blobs * n_sub;
+    unsigned blocks = (unsigned)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
+    if (prec == RPY_PREC_F64)
+        rpy::subdivide_kernel<double><<<blocks, 256, 0, st>>>((const double*)d_pos, (const double*)d_force, (const double*)d_template,
+                                                             (double*)d_sub_pos, (double*)d_sub_force, n_blobs, n_rhs, n_sub);
+    else
+        rpy::subdivide_kernel<float><<<blocks, 256, 0, st>>>((const float*)d_pos, (const float*)d_force, (const float*)d_template,
+                                                            (float*)d_sub_pos, (float*)d_sub_force, n_blobs, n_rhs, n_sub);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
 }
 
 rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos,
