@@ -309,7 +309,8 @@ def time_solve(torch, cfg: int, matvec_prec: str, tol: float, restart: int = 60)
     vec = torch.randn(b.n, dtype=torch.float64, device=dev)
     out = torch.empty_like(vec)
     apply_ms, _ = timed(lambda: rigid.rpy_rigid_precond_apply(pc, vec, out=out), reps=10)
-    saddle_ms, _ = timed(lambda: rigid.rpy_rigid_saddle_apply(b, vec, "wall", wl.a, wl.eta, matvec_prec), reps=3)
+    inner = "f32" if matvec_prec == "mixed" else matvec_prec
+    saddle_ms, _ = timed(lambda: rigid.rpy_rigid_saddle_apply(b, vec, "wall", wl.a, wl.eta, inner), reps=3)
     ws = torch.empty(rigid.rpy_rigid_solve_workspace_bytes(matvec_prec, b.n_blobs, b.n_bodies, restart),
                      dtype=torch.uint8, device=dev)
     solve = lambda: rigid.rpy_rigid_mobility_solve(b, pc, F, slip, "wall", wl.a, wl.eta, tol=tol, restart=restart,
@@ -434,7 +435,7 @@ def run_ours(args):
             line["other_configs"] = extra
             # --- next rows of SURVEY 8(f): the preconditioned GMRES mobility solve around the matvec
             solves = []
-            for cfg, p, tol in ((2, "f64", 1e-8), (3, "f64", 1e-8), (3, "f32", 1e-5)):
+            for cfg, p, tol in ((2, "f64", 1e-8), (2, "mixed", 1e-8), (3, "f64", 1e-8), (3, "mixed", 1e-8), (3, "f32", 1e-5)):
                 try:
                     solves.append(time_solve(torch, cfg, p, tol))
                     log(f"[bench] solve {solves[-1]}")

@@ -46,6 +46,14 @@ extern "C" {
  * non-positive pivot (a blob overlapping the wall, or coincident blobs). */
 #define RPY_ERR_NOT_SPD 6
 
+/* Third value of matvec_prec accepted by the solve only: fp32 products inside every GMRES cycle, an
+ * fp64 product for the residual each cycle starts from.  "Krylov methods ... allow one to lower the
+ * accuracy of the matrix-vector product as the residual is reduced": a cycle ends
+ * when its fp32 residual estimate has dropped by 1e-4 (or reached tol), x is updated, the true fp64
+ * residual of Eq. (11) is recomputed and decides convergence.  Reaches fp64 tolerances at mostly
+ * fp32 cost; *h_rel_resid is then the TRUE relative residual. */
+#define RPY_PREC_MIXED 2
+
 /* out[i] = beta * out[i] + alpha * (K U)_i.   beta == 0 overwrites (out may be uninitialised).
  *   d_pos [n_blobs][3], d_q [n_bodies][3], d_offsets [n_bodies+1] (int64), d_U [n_bodies][6],
  *   d_out [n_blobs][3] : device.  One warp per body.                                              */
@@ -93,6 +101,15 @@ rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void
 rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t *h_offsets, const void *d_precond,
                                  int64_t body, double *d_factor, double *d_body_mobility,
                                  void *cuda_stream);
+
+/* Blob positions of identical bodies from their poses (footnote 4: "only the positions
+ * and orientations of the rigid bodies (so only up to 7 numbers per body) need to be communicated to
+ * the GPU"):  r_{p,t} = c_p + R(theta_p) template_t,  blob index p * blobs_per_body + t.
+ *   d_template [blobs_per_body][3] reference configuration, d_centres [n_bodies][3],
+ *   d_quats [n_bodies][4] unit quaternions (s, p1, p2, p3) (normalised again inside),
+ *   d_pos [n_bodies * blobs_per_body][3] overwritten.  Element type per `prec` (double / float).   */
+rpy_status rpy_rigid_blob_positions(rpy_prec prec, int64_t n_bodies, int blobs_per_body, const void *d_template,
+                                    const void *d_centres, const void *d_quats, void *d_pos, void *cuda_stream);
 
 /* Workspace of the solve: restart+1 Krylov vectors, three work vectors, the matvec workspace and
  * (fp32 matvec) float copies of positions, iterate and product.                                   */

@@ -60,6 +60,23 @@ def KT_apply(pos, q, offsets, lam) -> np.ndarray:
     return out
 
 
+def blob_positions(template, centres, quats) -> np.ndarray:
+    """Blob positions of identical bodies from their poses (footnote 4; Eq. (1)'s
+    r_i = q + R (r_i^ref)): rotation by the unit quaternion theta = (s, p) applied as
+    v' = v + 2 s (p x v) + 2 p x (p x v)  (no rotation matrix is formed)."""
+    template = np.asarray(template, dtype=np.float64); centres = np.asarray(centres, dtype=np.float64)
+    quats = np.asarray(quats, dtype=np.float64)
+    out = np.zeros((centres.shape[0], template.shape[0], 3))
+    for b in range(centres.shape[0]):
+        th = quats[b] / np.linalg.norm(quats[b])
+        s, p = th[0], th[1:]
+        for t in range(template.shape[0]):
+            v = template[t]
+            pv = np.cross(p, v)
+            out[b, t] = centres[b] + v + 2.0 * s * pv + 2.0 * np.cross(p, pv)
+    return out.reshape(-1, 3)
+
+
 def K_matrix(pos, q, offsets) -> np.ndarray:
     """Dense K, (3 N_b) x (6 N_bodies): column c is K applied to the c-th unit motion."""
     pos, q, offsets, nb = _check(pos, q, offsets)

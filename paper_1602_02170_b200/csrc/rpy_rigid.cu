@@ -90,6 +90,28 @@ __global__ void kt_apply_kernel(const double* __restrict__ pos, const double* __
     }
 }
 
+// r = c_p + R(theta_p) t, R from the unit quaternion (s, p): the standard rotation matrix.
+template <class S>
+__global__ void blob_positions_kernel(const S* __restrict__ tmpl, const S* __restrict__ centres,
+                                      const S* __restrict__ quats, S* __restrict__ pos, int64_t n_bodies, int bpb)
+{
+    const int64_t total = n_bodies * bpb;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t p = e / bpb;
+        const int t = (int)(e % bpb);
+        double s = quats[4 * p + 0], x = quats[4 * p + 1], y = quats[4 * p + 2], z = quats[4 * p + 3];
+        const double nrm = 1.0 / sqrt(s * s + x * x + y * y + z * z);
+        s *= nrm; x *= nrm; y *= nrm; z *= nrm;
+        const double tx = tmpl[3 * t + 0], ty = tmpl[3 * t + 1], tz = tmpl[3 * t + 2];
+        const double rx = (1 - 2 * (y * y + z * z)) * tx + 2 * (x * y - s * z) * ty + 2 * (x * z + s * y) * tz;
+        const double ry = 2 * (x * y + s * z) * tx + (1 - 2 * (x * x + z * z)) * ty + 2 * (y * z - s * x) * tz;
+        const double rz = 2 * (x * z - s * y) * tx + 2 * (y * z + s * x) * ty + (1 - 2 * (x * x + y * y)) * tz;
+        pos[3 * e + 0] = (S)((double)centres[3 * p + 0] + rx);
+        pos[3 * e + 1] = (S)((double)centres[3 * p + 1] + ry);
+        pos[3 * e + 2] = (S)((double)centres[3 * p + 2] + rz);
+    }
+}
+
 // ------------------------------------------------------------------ preconditioner storage
 // [header 4 x int64][offsets nb+1][mat_off nb+1][info nb x int32][factors][Y 3N x 6][Nt nb x 36]
 struct PrecondLayout {
@@ -577,6 +599,9 @@ rpy_status check_bodies(int64_t n_blobs, int64_t n_bodies)
     return RPY_OK;
 }
 
+constexpr rpy_prec kPrecMixed = static_cast<rpy_prec>(RPY_PREC_MIXED);
+constexpr double kInnerReduction = 1e-4;     // residual reduction asked of one fp32 cycle (mixed solve)
+
 // Solver workspace, carved from one caller-owned buffer.
 struct SolveWs {
     int64_t n; size_t vec_bytes;
@@ -606,11 +631,14 @@ SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, voi
     W.st.yv = (double*)take((size_t)restart * 8); W.st.scal = (double*)take(8 * 8);
     W.partial = (double*)take((size_t)kVecBlocks * (restart + 1) * 8);
     W.norm_partial = (double*)take((size_t)kVecBlocks * 8);
-    if (prec == RPY_PREC_F32_ACC64) {
+    if (prec != RPY_PREC_F64) {
         W.pos32 = (float*)take((size_t)n_blobs * 12); W.lam32 = (float*)take((size_t)n_blobs * 12);
         W.vel32 = (float*)take((size_t)n_blobs * 12);
     } else { W.pos32 = W.lam32 = W.vel32 = nullptr; }
-    W.mv_bytes = rpy_matvec_workspace_bytes(prec, n_blobs, 1);
+    W.mv_bytes = prec == kPrecMixed
+        ? (rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, 1) > rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, 1)
+               ? rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, 1) : rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, 1))
+        : rpy_matvec_workspace_bytes(prec, n_blobs, 1);
     W.mv = take(W.mv_bytes);
     W.total = at;
     return W;
@@ -678,6 +706,26 @@ rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double* d
     if (!isfinite(alpha) || !isfinite(beta)) return RPY_ERR_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     kt_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_lambda, alpha, beta, d_out, n_bodies);
+    RPY_CUDA_TRY(cudaGetLastError());
+    return RPY_OK;
+}
+
+rpy_status rpy_rigid_blob_positions(rpy_prec prec, int64_t n_bodies, int blobs_per_body, const void* d_template,
+                                    const void* d_centres, const void* d_quats, void* d_pos, void* cuda_stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n_bodies < 0 || blobs_per_body < 1 || n_bodies * (int64_t)blobs_per_body > RPY_MAX_BLOBS) return RPY_ERR_ARG;
+    if (n_bodies == 0) return RPY_OK;
+    if (!d_template || !d_centres || !d_quats || !d_pos) return RPY_ERR_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t total = n_bodies * blobs_per_body;
+    const unsigned blocks = (unsigned)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
+    if (prec == RPY_PREC_F64)
+        blob_positions_kernel<double><<<blocks, 256, 0, st>>>((const double*)d_template, (const double*)d_centres,
+                                                             (const double*)d_quats, (double*)d_pos, n_bodies, blobs_per_body);
+    else
+        blob_positions_kernel<float><<<blocks, 256, 0, st>>>((const float*)d_template, (const float*)d_centres,
+                                                            (const float*)d_quats, (float*)d_pos, n_bodies, blobs_per_body);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -813,7 +861,7 @@ rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t* h_offsets, con
 
 size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart)
 {
-    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64) return 0;
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return 0;
     if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1 || restart < 1 || restart > RPY_RIGID_MAX_RESTART) return 0;
     return carve(matvec_prec, n_blobs, n_bodies, restart, nullptr).total;
 }
@@ -843,7 +891,10 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
                                     double* h_history, int* h_n_iter, double* h_rel_resid,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return RPY_ERR_ARG;
+    const bool mixed = matvec_prec == kPrecMixed;
+    const rpy_prec inner_prec = mixed ? RPY_PREC_F32_ACC64 : matvec_prec;     // the product inside Arnoldi
+    const rpy_prec outer_prec = mixed ? RPY_PREC_F64 : matvec_prec;           // the product of a restart's residual
     if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1) return RPY_ERR_ARG;
     if (!finite_pos(a) || !finite_pos(eta) || !(tol >= 0.0) || restart < 1 || restart > RPY_RIGID_MAX_RESTART || max_iter < 1)
         return RPY_ERR_ARG;
@@ -856,7 +907,7 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
     int64_t bad = -1;
     rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
     if (s != RPY_OK) return s;
-    if (matvec_prec == RPY_PREC_F32_ACC64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * N);
+    if (matvec_prec != RPY_PREC_F64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * N);
 
     // b = [slip; -F], x = 0, r0 = b
     if (d_slip) RPY_CUDA_TRY(cudaMemcpyAsync(W.b, d_slip, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
@@ -880,13 +931,14 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
     }
     const double* r = W.b;
     bool done = false;
+    double beta_cycle = bnorm;                   // norm of the residual the current cycle starts from
     while (!done) {
         scale_kernel<<<kVecBlocks, 256, 0, st>>>(r, W.st.scal + 1, W.V, n);          // v_0 = r / beta
         int k = 0;
         for (int j = 0; j < restart; ++j) {
             const double* vj = W.V + (int64_t)j * ldv;
             if ((s = precond_apply(N, nb, d_precond, vj, W.z, st)) != RPY_OK) return s;
-            if ((s = saddle(wall, matvec_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, W, st)) != RPY_OK) return s;
+            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, W, st)) != RPY_OK) return s;
             ++n_iter;
             // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
             dots_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial);
@@ -901,7 +953,11 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
             rel = res / bnorm;
             if (h_history) h_history[n_iter] = rel;
             k = j + 1;
-            if (!(rel > tol) || n_iter >= max_iter) { done = true; break; }
+            if (mixed) {
+                // the estimate is the residual of the fp32 operator: end the cycle once it has gained
+                // kInnerReduction (or reached tol) and let the fp64 residual below decide
+                if (!(rel > tol) || !(res > kInnerReduction * beta_cycle) || n_iter >= max_iter) break;
+            } else if (!(rel > tol) || n_iter >= max_iter) { done = true; break; }
         }
         // x += P^-1 (V_k y),  R y = g
         solve_y_kernel<<<1, 32, 0, st>>>(W.st, k, W.ldr);
@@ -909,12 +965,19 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
         if ((s = precond_apply(N, nb, d_precond, W.w, W.z, st)) != RPY_OK) return s;
         axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.z, 1.0, W.x, n);
         if (done) break;
-        // restart: r = b - A x
-        if ((s = saddle(wall, matvec_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, W, st)) != RPY_OK) return s;
+        // restart: r = b - A x  (mixed solve: with the fp64 product -- the true residual of Eq. (11))
+        if ((s = saddle(wall, outer_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, W, st)) != RPY_OK) return s;
         axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.b, -1.0, W.w, n);
         norm_partial_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.w, n, W.norm_partial);
         cycle_start_kernel<<<1, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, restart, 0);
         r = W.w;
+        if (mixed) {
+            RPY_CUDA_TRY(cudaMemcpyAsync(&beta_cycle, W.st.scal, 8, cudaMemcpyDeviceToHost, st));
+            RPY_CUDA_TRY(cudaStreamSynchronize(st));
+            rel = beta_cycle / bnorm;
+            if (h_history) h_history[n_iter] = rel;                 // replace the estimate by the true value
+            if (!(rel > tol) || n_iter >= max_iter) done = true;
+        }
     }
     RPY_CUDA_TRY(cudaMemcpyAsync(d_lambda, W.x, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
     RPY_CUDA_TRY(cudaMemcpyAsync(d_U, W.x + 3 * N, (size_t)nb * 48, cudaMemcpyDeviceToDevice, st));

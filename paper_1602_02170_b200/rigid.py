@@ -17,6 +17,7 @@ from . import binding
 from .binding import RPY_PREC_F64, RPY_PREC_F32_ACC64, RpyError, _prec_code  # noqa: F401
 
 RPY_ERR_NOT_SPD = 6
+RPY_PREC_MIXED = 2       # solve only: fp32 products inside a cycle, fp64 residual per cycle
 RPY_RIGID_MAX_BODY_BLOBS = 512
 RPY_RIGID_MAX_RESTART = 128
 
@@ -26,6 +27,7 @@ _i64p, _dblp, _intp = ctypes.POINTER(_i64), ctypes.POINTER(_dbl), ctypes.POINTER
 SIGNATURES = {
     "rpy_rigid_K_apply": (_int, [_i64, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp]),
     "rpy_rigid_KT_apply": (_int, [_i64, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp]),
+    "rpy_rigid_blob_positions": (_int, [_int, _i64, _int, _vp, _vp, _vp, _vp, _vp]),
     "rpy_rigid_precond_bytes": (_sz, [_i64, _i64p]),
     "rpy_rigid_precond_build": (_int, [_int, _i64, _i64, _vp, _vp, _i64p, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_rigid_precond_info": (_int, [_i64, _vp, _i64p, _vp]),
@@ -133,6 +135,23 @@ def rpy_rigid_KT_apply(b: Bodies, lam: torch.Tensor, alpha: float = 1.0, beta: f
     return out
 
 
+def rpy_rigid_blob_positions(template: torch.Tensor, centres: torch.Tensor, quats: torch.Tensor) -> torch.Tensor:
+    """Blob positions [n_bodies * blobs_per_body, 3] of identical bodies from their poses:
+    r = c_p + R(theta_p) template_t, quaternions (s, p1, p2, p3).  float64 or float32 CUDA tensors."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("the rigid layer needs a CUDA device (sm_100a); there is no CPU fallback")
+    nb, bpb = centres.shape[0], template.shape[0]
+    for t, shape, what in ((template, (bpb, 3), "template"), (centres, (nb, 3), "centres"), (quats, (nb, 4), "quats")):
+        if not t.is_cuda or t.dtype != template.dtype or not t.is_contiguous() or tuple(t.shape) != shape:
+            raise ValueError(f"{what} must be a contiguous CUDA tensor of shape {shape} and the template's dtype")
+    pos = torch.empty((nb * bpb, 3), dtype=template.dtype, device=template.device)
+    with torch.cuda.device(template.device):
+        _check(_lib().rpy_rigid_blob_positions(binding._prec_of(template.dtype), nb, bpb, template.data_ptr(),
+                                               centres.data_ptr() or None, quats.data_ptr() or None,
+                                               pos.data_ptr() or None, _stream(template)))
+    return pos
+
+
 def _hptr(h: torch.Tensor):
     return ctypes.cast(h.data_ptr(), _i64p)
 
@@ -205,7 +224,8 @@ def rpy_rigid_precond_get(pc: Precond, body: int):
 
 
 def rpy_rigid_solve_workspace_bytes(matvec_prec, n_blobs: int, n_bodies: int, restart: int) -> int:
-    return int(_lib().rpy_rigid_solve_workspace_bytes(_prec_code(matvec_prec), int(n_blobs), int(n_bodies), int(restart)))
+    prec = RPY_PREC_MIXED if matvec_prec in ("mixed", RPY_PREC_MIXED) else _prec_code(matvec_prec)
+    return int(_lib().rpy_rigid_solve_workspace_bytes(prec, int(n_blobs), int(n_bodies), int(restart)))
 
 
 def rpy_rigid_saddle_apply(b: Bodies, x: torch.Tensor, variant: str = "wall", a: float = 1.0, eta: float = 1.0,
@@ -231,7 +251,7 @@ def rpy_rigid_mobility_solve(b: Bodies, pc: Precond, F: torch.Tensor, slip: Opti
     _f64(F, (b.n_bodies, 6), "F")
     if slip is not None:
         _f64(slip, (b.n_blobs, 3), "slip")
-    prec = _prec_code(matvec_prec)
+    prec = RPY_PREC_MIXED if matvec_prec in ("mixed", RPY_PREC_MIXED) else _prec_code(matvec_prec)
     need = rpy_rigid_solve_workspace_bytes(prec, b.n_blobs, b.n_bodies, restart)
     if need == 0:
         raise ValueError("invalid sizes or restart length")

@@ -121,3 +121,26 @@ def test_preconditioner_is_exact_for_one_body_and_block_diagonal_otherwise():
         sp = slice(b.offsets[p], b.offsets[p + 1])
         r = Mpp @ lam[sp].reshape(-1) - rigid.K_apply(w.pos[sp], b.q[p:p + 1], np.array([0, 15]), U[p:p + 1]).reshape(-1)
         assert np.allclose(r, x[sp].reshape(-1), atol=1e-10)
+
+
+def test_blob_positions_from_poses_by_hand_and_by_group_properties():
+    """Footnote 4.  Quarter turns computed by hand; rotations preserve lengths; the
+    quaternion product composes rotations; the seeded generator's own matrix form agrees."""
+    tmpl = np.array([[1.0, 0, 0], [0, 2.0, 0], [0, 0, 3.0]])
+    c = np.array([[10.0, 20.0, 30.0]])
+    h = np.sqrt(0.5)
+    # quarter turn about z: x -> y, y -> -x
+    out = rigid.blob_positions(tmpl, c, np.array([[h, 0, 0, h]]))
+    assert np.allclose(out, c + np.array([[0, 1.0, 0], [-2.0, 0, 0], [0, 0, 3.0]]), atol=1e-15)
+    # quarter turn about x: y -> z, z -> -y ; an unnormalised quaternion gives the same rotation
+    out = rigid.blob_positions(tmpl, c, np.array([[3.0, 3.0, 0, 0]]))
+    assert np.allclose(out, c + np.array([[1.0, 0, 0], [0, 0, 2.0], [0, -3.0, 0]]), atol=1e-14)
+    rng = np.random.default_rng(0)
+    q1, q2 = rng.standard_normal(4), rng.standard_normal(4)
+    q1 /= np.linalg.norm(q1); q2 /= np.linalg.norm(q2)
+    q12 = np.concatenate([[q1[0] * q2[0] - q1[1:] @ q2[1:]], q1[0] * q2[1:] + q2[0] * q1[1:] + np.cross(q1[1:], q2[1:])])
+    t = rng.standard_normal((5, 3)); z = np.zeros((1, 3))
+    two = rigid.blob_positions(rigid.blob_positions(t, z, q2[None]), z, q1[None])
+    assert np.allclose(two, rigid.blob_positions(t, z, q12[None]), atol=1e-14)
+    assert np.allclose(np.linalg.norm(two, axis=1), np.linalg.norm(t, axis=1))
+    assert np.allclose(rigid.blob_positions(t, c, q1[None]), t @ workloads.quat_to_rot(q1[None])[0].T + c, atol=1e-14)

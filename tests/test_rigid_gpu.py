@@ -205,3 +205,45 @@ def test_config2_full_size_solve_residual_checked_by_the_oracle():
     res = np.sqrt(np.sum(top ** 2) + np.sum(bot ** 2)) / bn
     print(f"cfg2 solve: {r['n_iter']} iterations, estimated residual {r['rel_resid']:.2e}, oracle residual {res:.2e}")
     assert res <= 2e-8 and r["n_iter"] <= 50      # measured: 43 (Table III's range: 7-43)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_blob_positions_from_poses_and_matvec_equals_explicit_position_path(prec):
+    """Footnote 4: 7 numbers per body cross the bus; the matvec on the generated
+    positions equals the matvec on explicitly supplied positions."""
+    from paper_1602_02170_b200 import binding
+    npdt = np.float64 if prec == "f64" else np.float32
+    rng = np.random.default_rng(11)
+    nb = 300
+    tmpl = (3.0 * workloads.shell_template(42)).astype(npdt)
+    quats = rng.standard_normal((nb, 4)).astype(npdt)
+    centres = np.stack([rng.uniform(0, 200, nb), rng.uniform(0, 200, nb), rng.uniform(4.2, 9, nb)], 1).astype(npdt)
+    pos = rigid.rpy_rigid_blob_positions(torch.from_numpy(tmpl).cuda(), torch.from_numpy(centres).cuda(),
+                                         torch.from_numpy(quats).cuda())
+    ref = origid.blob_positions(tmpl.astype(np.float64), centres.astype(np.float64), quats.astype(np.float64))
+    err = np.abs(pos.cpu().numpy().astype(np.float64) - ref).max()
+    assert err <= (1e-13 if prec == "f64" else 2e-5)          # coordinates up to 200: ~1 ulp of the output type
+    lam = torch.from_numpy(rng.standard_normal((nb * 42, 3)).astype(npdt)).cuda()
+    u_pose = binding.rpy_wall_matvec(pos, lam)
+    u_expl = binding.rpy_wall_matvec(pos.clone(), lam)
+    assert torch.equal(u_pose, u_expl) or rel(u_pose.cpu().numpy(), u_expl.cpu().numpy()) < 1e-13   # atomics order
+    uo = oracle.matvec(oracle.WALL, pos.cpu().numpy().astype(np.float64), lam.cpu().numpy().astype(np.float64))
+    assert rel(u_pose.cpu().numpy().astype(np.float64), uo) <= (1e-12 if prec == "f64" else 1e-5)
+
+
+def test_mixed_precision_solve_reaches_fp64_tolerance_with_fp32_products():
+    """the product's accuracy may be lowered inside the Krylov solve.  fp32 products in
+    every cycle, fp64 residual per cycle: same answer as the dense solve, true residual <= tol."""
+    pos, b, lam, db = boomerangs(60, seed=9)
+    slip = 0.1 * np.random.default_rng(3).standard_normal(pos.shape)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    lam_d, U_d = origid.mobility_solve(oracle.WALL, pos, b.q, b.offsets, b.F, slip)
+    r = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=1e-9, matvec_prec="mixed")
+    assert r["rel_resid"] <= 1e-9
+    assert rel(r["U"].cpu().numpy(), U_d) < 1e-7 and rel(r["lambda"].cpu().numpy(), lam_d) < 1e-6
+    x = torch.cat([r["lambda"].reshape(-1), r["U"].reshape(-1)])
+    res = rigid.rpy_rigid_saddle_apply(db, x, "wall").cpu().numpy() - np.concatenate([slip.ravel(), -b.F.ravel()])
+    assert np.linalg.norm(res) / np.sqrt(np.sum(slip ** 2) + np.sum(b.F ** 2)) <= 1.001e-9
+    full = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=1e-9)
+    print(f"mixed: {r['n_iter']} fp32 iterations; fp64: {full['n_iter']} iterations")
+    assert r["n_iter"] <= 2 * full["n_iter"] + 4
