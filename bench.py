@@ -461,11 +461,21 @@ def main():
     ap.add_argument("--variant", choices=["wall", "free"], default="wall")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configurations")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing")
+    ap.add_argument("--rigid-solve", type=int, default=0, choices=[0, 2, 3],
+                    help="only time the preconditioned GMRES mobility solve on this rigid-body config "
+                         "(--prec f64|f32, or --solve-prec mixed) and print its JSON (profiling aid)")
+    ap.add_argument("--solve-prec", choices=["f64", "f32", "mixed"], default="f64")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         log("[bench] note: fewer than 3 warm-up steps requested")
     if args.impl == "reference":
         return run_reference(args)
+    if args.rigid_solve:
+        import torch
+        torch.cuda.set_device(0)
+        tol = 1e-5 if args.solve_prec == "f32" else 1e-8
+        print(json.dumps(time_solve(torch, args.rigid_solve, args.solve_prec, tol)), flush=True)
+        return 0
     return run_ours(args)
 
 
