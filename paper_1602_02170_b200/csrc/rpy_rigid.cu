@@ -191,9 +191,9 @@ __device__ __forceinline__ void pair_block(double xi, double yi, double zi, doub
 // ------------------------------------------------------------------ preconditioner build
 // One CTA per body.  A (m x m, leading dimension ld) is in shared memory when m <= kSmemBodyM, else
 // it is the body's slot of `factors` (ld = m).  Steps: fill M^(pp); right-looking Cholesky on the
-// lower triangle, one barrier per column (thread t owns trailing columns k = j+1+t, ...: its
-// multiplier A[k][j] stays in a register, A[i][j] is a broadcast read, A[i][k] is conflict-free /
-// coalesced across threads); Y = (L L^T)^-1 K_p, one warp per column of K_p; N~ = (K_p^T Y)^-1 by
+// lower triangle, one barrier per column (the 256 threads tile the trailing triangle 16 x 16:
+// thread (tx, ty) updates A[i][k] for i = j+1+ty+16a, k = j+1+tx+16b <= i; a half-warp touches 16
+// consecutive doubles of one row); Y = (L L^T)^-1 K_p, one warp per column of K_p; N~ = (K_p^T Y)^-1 by
 // Gauss-Jordan on the 6x6; store L mirrored into both triangles.
 template <bool WALL>
 __global__ void __launch_bounds__(kBuildThreads)
@@ -206,6 +206,7 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
     __shared__ double s_n[36];
     __shared__ int s_fail;
     const int p = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tx = tid & 15, ty = tid >> 4;
     const int64_t b0 = offsets[p];
     const int nbp = (int)(offsets[p + 1] - b0);
     const int m = 3 * nbp;
@@ -233,9 +234,19 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
         const double d = A[(size_t)j * ld + j];
         if (!(d > 0.0) || !isfinite(d)) { if (tid == 0) s_fail = j + 1; break; }   // uniform: all threads read the same d
         const double rd = 1.0 / d;
-        for (int k = j + 1 + tid; k < m; k += kBuildThreads) {
-            const double ckj = A[(size_t)k * ld + j] * rd;
-            for (int i = k; i < m; ++i) A[(size_t)i * ld + k] -= A[(size_t)i * ld + j] * ckj;
+        // trailing update A[i][k] -= A[i][j] A[k][j] / d for j < k <= i: 16 x 16 thread tile over (i, k)
+        for (int i = j + 1 + ty; i < m; i += 16) {
+            const double lij = A[(size_t)i * ld + j] * rd;
+            double* Ai = A + (size_t)i * ld;
+            int k = j + 1 + tx;
+            for (; k + 48 <= i; k += 64) {           // four independent load-FMA-store chains in flight
+                const double c0 = A[(size_t)k * ld + j], c1 = A[(size_t)(k + 16) * ld + j];
+                const double c2 = A[(size_t)(k + 32) * ld + j], c3 = A[(size_t)(k + 48) * ld + j];
+                const double a0 = Ai[k], a1 = Ai[k + 16], a2 = Ai[k + 32], a3 = Ai[k + 48];
+                Ai[k] = a0 - lij * c0; Ai[k + 16] = a1 - lij * c1;
+                Ai[k + 32] = a2 - lij * c2; Ai[k + 48] = a3 - lij * c3;
+            }
+            for (; k <= i; k += 16) Ai[k] -= lij * A[(size_t)k * ld + j];
         }
         __syncthreads();
         const double rs = 1.0 / sqrt(d);
@@ -325,46 +336,13 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
 // The right-hand side lives in the warp's slice of `out` (each warp touches only its own body's
 // entries); row j of the stored factor holds column j of L to the right of the diagonal and row j of
 // L to its left, so both substitutions read one contiguous row per step.
-__global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
-                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies)
+constexpr int kApplySmallM = 63;                 // bodies up to 21 blobs: factor staged in shared memory
+constexpr int kApplySmallWarpDoubles = 4096;     // 63 * 63 + 63 <= 4096 doubles = 32 KB per warp
+constexpr int kApplySmallWarps = 2;              // 64 KB per CTA, three CTAs per SM
+
+// t <- (L L^T)^-1 t for one body by one warp; S is the stored factor (leading dimension m).
+__device__ __forceinline__ void warp_substitutions(const double* S, double* t, int m, int lane)
 {
-    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    const int64_t* hdr = static_cast<const int64_t*>(precond);
-    if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
-    const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
-    const int64_t* offsets = pv.offsets;
-    const int64_t* mat_off = pv.mat_off;
-    const double* factors = pv.factors;
-    const double* Yg = pv.Y;
-    const double* Ntg = pv.Nt;
-    const int64_t b0 = offsets[p];
-    const int m = 3 * (int)(offsets[p + 1] - b0);
-    const double* S = factors + mat_off[p];
-    const double* Y = Yg + b0 * 18;
-    const double* x = in + 3 * b0;
-    const double* y = in + 3 * n_blobs + 6 * p;
-    double* t = out + 3 * b0;
-
-    double r[6] = {0, 0, 0, 0, 0, 0};
-    for (int i = lane; i < m; i += 32) {
-        const double xi = x[i];
-        t[i] = xi;
-#pragma unroll
-        for (int c = 0; c < 6; ++c) r[c] += Y[(size_t)i * 6 + c] * xi;
-    }
-#pragma unroll
-    for (int c = 0; c < 6; ++c) r[c] = warp_sum(r[c]) + y[c];
-    double U[6];
-#pragma unroll
-    for (int a = 0; a < 6; ++a) {
-        double s = 0.0;
-#pragma unroll
-        for (int c = 0; c < 6; ++c) s += Ntg[(size_t)p * 36 + 6 * a + c] * r[c];
-        U[a] = -s;
-    }
-    __syncwarp();
-
     // forward: for j = 0..m-1: t_j /= L_jj; t_i -= L_ij t_j (i > j); L_ij = S[j][i]
     for (int j = 0; j < m; ++j) {
         const double* row = S + (size_t)j * m;
@@ -383,8 +361,60 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
         for (int i = lane; i < j; i += 32) t[i] -= row[i] * tj;
         __syncwarp();
     }
+}
+
+// SMALL = true: handles the bodies with 3*blobs <= kApplySmallM -- the warp first copies the whole
+// factor (<= 31 KB) and the right-hand side into its slice of shared memory, so the 2m dependent
+// substitution steps run at shared-memory latency; larger bodies are skipped.  SMALL = false: the
+// other bodies, factor rows read from L2/HBM, right-hand side in the warp's slice of `out`.
+template <bool SMALL>
+__global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
+                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies)
+{
+    extern __shared__ __align__(16) double sm_apply[];
+    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    const int64_t* hdr = static_cast<const int64_t*>(precond);
+    if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
+    const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
+    const int64_t b0 = pv.offsets[p];
+    const int m = 3 * (int)(pv.offsets[p + 1] - b0);
+    if ((m <= kApplySmallM) != SMALL) return;
+    const double* S = pv.factors + pv.mat_off[p];
+    const double* Y = pv.Y + b0 * 18;
+    const double* Ntg = pv.Nt;
+    const double* x = in + 3 * b0;
+    const double* y = in + 3 * n_blobs + 6 * p;
+    double* t = out + 3 * b0;
+    double* ts = t;                      // where the substitutions work
+    if (SMALL) {
+        double* mine = sm_apply + (size_t)(threadIdx.x >> 5) * kApplySmallWarpDoubles;
+        for (int e = lane; e < m * m; e += 32) mine[e] = S[e];
+        S = mine;
+        ts = mine + m * m;
+    }
+
+    double r[6] = {0, 0, 0, 0, 0, 0};
     for (int i = lane; i < m; i += 32) {
-        double s = t[i];
+        const double xi = x[i];
+        ts[i] = xi;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) r[c] += Y[(size_t)i * 6 + c] * xi;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) r[c] = warp_sum(r[c]) + y[c];
+    double U[6];
+#pragma unroll
+    for (int a = 0; a < 6; ++a) {
+        double s = 0.0;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) s += Ntg[(size_t)p * 36 + 6 * a + c] * r[c];
+        U[a] = -s;
+    }
+    __syncwarp();
+    warp_substitutions(S, ts, m, lane);
+    for (int i = lane; i < m; i += 32) {
+        double s = ts[i];
 #pragma unroll
         for (int c = 0; c < 6; ++c) s += Y[(size_t)i * 6 + c] * U[c];
         t[i] = s;
@@ -438,11 +468,14 @@ update_kernel(const double* __restrict__ V, int64_t ldv, int nvec, double* __res
 {
     __shared__ double h[RPY_RIGID_MAX_RESTART + 1];
     __shared__ double red[kVecThreads / 32];
-    for (int v = threadIdx.x; v < nvec; v += kVecThreads) {
+    for (int v = threadIdx.x >> 5; v < nvec; v += kVecThreads / 32) {      // one warp per dot product
         double s = 0.0;
-        for (int b = 0; b < (int)gridDim.x; ++b) s += partial[(int64_t)v * gridDim.x + b];
-        h[v] = s;
-        if (blockIdx.x == 0) hcol[v] = (accumulate ? hcol[v] : 0.0) + s;
+        for (int b = threadIdx.x & 31; b < (int)gridDim.x; b += 32) s += partial[(int64_t)v * gridDim.x + b];
+        s = warp_sum(s);
+        if ((threadIdx.x & 31) == 0) {
+            h[v] = s;
+            if (blockIdx.x == 0) hcol[v] = (accumulate ? hcol[v] : 0.0) + s;
+        }
     }
     __syncthreads();
     int64_t lo, hi; chunk_of(n, lo, hi);
@@ -478,9 +511,10 @@ struct GmresState {
 // earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").
 __global__ void hessenberg_kernel(GmresState st, int j, int ldr, const double* __restrict__ norm_partial, int nblk)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    double s = 0.0;
-    for (int b = 0; b < nblk; ++b) s += norm_partial[b];
+    double s = 0.0;                                  // one warp: fixed-order strided sums, then shuffles
+    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[b];
+    s = warp_sum(s);
+    if (threadIdx.x != 0) return;
     const double hn = sqrt(s);
     st.scal[0] = hn;
     st.scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
@@ -505,9 +539,10 @@ __global__ void hessenberg_kernel(GmresState st, int j, int ldr, const double* _
 // with set_bnorm, scal[3] = beta (the first cycle starts from x0 = 0, so r0 = b).
 __global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int restart, int set_bnorm)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double s = 0.0;
-    for (int b = 0; b < nblk; ++b) s += norm_partial[b];
+    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[b];
+    s = warp_sum(s);
+    if (threadIdx.x != 0) return;
     const double beta = sqrt(s);
     st.scal[0] = beta; st.scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; st.scal[2] = beta;
     if (set_bnorm) st.scal[3] = beta;
@@ -671,7 +706,12 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
 
 rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, cudaStream_t st)
 {
-    precond_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
+    // two launches, each warp decides from its body's size which of them serves it (no host state)
+    constexpr int small_threads = 32 * kApplySmallWarps;
+    constexpr int small_smem = kApplySmallWarps * kApplySmallWarpDoubles * 8;
+    RPY_CUDA_TRY(cudaFuncSetAttribute(precond_apply_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, small_smem));
+    precond_apply_kernel<true><<<warp_grid(nb, small_threads), small_threads, small_smem, st>>>(precond, in, out, N, nb);
+    precond_apply_kernel<false><<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
