@@ -13,8 +13,9 @@
  *               tau_p = sum_i (r_i - q_p) x lambda_i                       Eq. (10)
  *   P^-1        the indefinite block-diagonal preconditioner of Eq. (18): solve Eq. (19),
  *               [M~ -K; -K^T 0][lambda; U] = [x; y], with M~ the diagonal blocks M^(pp) of Eq. (17)
- *               (each body alone, with or without the wall), through a dense Cholesky
- *               factorisation of every M^(pp) and the 6x6 body mobilities
+ *               (each body alone, with or without the wall), through the dense inverse of every
+ *               M^(pp), formed from its Cholesky factor ("dense matrix inversion (e.g., Cholesky
+ *               factorization)"), and the 6x6 body mobilities
  *               N~_pp = (K_p^T (M^(pp))^-1 K_p)^-1
  *   solve       Eq. (11), [M -K; -K^T 0][lambda; U] = [slip; -F], by right-preconditioned
  *               restarted GMRES
@@ -69,13 +70,13 @@ rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double *d
 
 /* Bytes of device memory the preconditioner of these bodies needs (host arithmetic on the HOST
  * array h_offsets [n_bodies+1]); 0 if the offsets are not a valid partition.  Per body with
- * m = 3 * blobs: m*m doubles (Cholesky factor L in the lower triangle AND L^T in the upper one, so
- * both substitutions read contiguous rows), m*6 (Y = (M^(pp))^-1 K_p), 36 (N~_pp), plus tables.  */
+ * m = 3 * blobs: m*m doubles (the full symmetric inverse of M^(pp)), m*6 (Y = (M^(pp))^-1 K_p),
+ * 36 (N~_pp), plus tables.  */
 size_t rpy_rigid_precond_bytes(int64_t n_bodies, const int64_t *h_offsets);
 
 /* Builds the preconditioner: for every body the dense M^(pp) (wall != 0: wall-corrected tensor,
- * else free space -- the "unbounded" preconditioner of Table III), its Cholesky
- * factor, Y and N~_pp.  One CTA per body; the matrix lives in shared memory when 3*blobs <= 162,
+ * else free space -- the "unbounded" preconditioner of Table III), its inverse
+ * (Cholesky factorisation, then L^-1 and L^-T L^-1 in place), Y and N~_pp.  One CTA per body; the matrix lives in shared memory when 3*blobs <= 162,
  * else in its slot of d_precond.  h_offsets is read before the call returns.
  * d_precond: device, 256-byte aligned, >= rpy_rigid_precond_bytes().  Synchronises the stream once (after
  * copying the offset tables up, before the build kernel is enqueued); a failed
@@ -85,21 +86,21 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
                                    void *d_precond, size_t precond_bytes, void *cuda_stream);
 
 /* Synchronises the stream and writes to *h_first_bad_body the smallest body index whose
- * factorisation failed, or -1.  Returns RPY_ERR_NOT_SPD in the former case.                        */
+ * factorisation (or 6x6 inversion) failed, or -1.  Returns RPY_ERR_NOT_SPD in the former case.                        */
 rpy_status rpy_rigid_precond_info(int64_t n_bodies, const void *d_precond, int64_t *h_first_bad_body,
                                   void *cuda_stream);
 
 /* [lambda; U] = P^-1 [x; y]: Eq. (19) for every body.  d_in, d_out: solver vectors
  * (3 n_blobs + 6 n_bodies doubles), d_out must not overlap d_in.  One warp per body:
- * t = (M^(pp))^-1 x by two triangular substitutions, U = -N~ (y + Y^T x), lambda = t + Y U.      */
+ * t = (M^(pp))^-1 x (dense symmetric product), U = -N~ (y + Y^T x), lambda = t + Y U.            */
 rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void *d_precond,
                                    const double *d_in, double *d_out, void *cuda_stream);
 
-/* Copies out pieces of a built preconditioner (tests, diagnostics): for body p, the factor
- * (row-major m x m, L in the lower triangle, L^T mirrored above) to d_factor if non-NULL, and the
- * 6x6 N~_pp (row-major) to d_body_mobility if non-NULL.  Device to device, stream ordered.        */
+/* Copies out pieces of a built preconditioner (tests, diagnostics): for body p, the inverse
+ * (M^(pp))^-1 (row-major m x m, symmetric) to d_inverse if non-NULL, and the 6x6 N~_pp (row-major)
+ * to d_body_mobility if non-NULL.  Device to device, stream ordered.                               */
 rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t *h_offsets, const void *d_precond,
-                                 int64_t body, double *d_factor, double *d_body_mobility,
+                                 int64_t body, double *d_inverse, double *d_body_mobility,
                                  void *cuda_stream);
 
 /* Blob positions of identical bodies from their poses (footnote 4: "only the positions

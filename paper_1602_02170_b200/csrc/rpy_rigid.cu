@@ -6,9 +6,9 @@
 // Kernels:
 //   k_apply / kt_apply        one warp per body; O(N_b)
 //   precond_build             one CTA per body: dense M^(pp) from the same pair arithmetic as the
-//                             matvec (rpy_math.cuh, double lanes), in-place Cholesky, Y = M^-1 K,
-//                             N~ = (K^T Y)^-1
-//   precond_apply             one warp per body: two triangular substitutions + 6x6 work
+//                             matvec (rpy_math.cuh, double lanes), in-place Cholesky, explicit inverse
+//                             from the factor, Y = M^-1 K, N~ = (K^T Y)^-1
+//   precond_apply             one warp per body: symmetric matrix-vector product + 6x6 work
 //   dots / update / hessenberg / scale / combine      the Krylov vector operations of GMRES
 #include <cuda_runtime.h>
 #include <math.h>
@@ -193,8 +193,8 @@ __device__ __forceinline__ void pair_block(double xi, double yi, double zi, doub
 // it is the body's slot of `factors` (ld = m).  Steps: fill M^(pp); right-looking Cholesky on the
 // lower triangle, one barrier per column (the 256 threads tile the trailing triangle 16 x 16:
 // thread (tx, ty) updates A[i][k] for i = j+1+ty+16a, k = j+1+tx+16b <= i; a half-warp touches 16
-// consecutive doubles of one row); Y = (L L^T)^-1 K_p, one warp per column of K_p; N~ = (K_p^T Y)^-1 by
-// Gauss-Jordan on the 6x6; store L mirrored into both triangles.
+// consecutive doubles of one row); the inverse (M^(pp))^-1 = L^-T L^-1 formed in place from the factor;
+// Y = (M^(pp))^-1 K_p; N~ = (K_p^T Y)^-1 by Gauss-Jordan on the 6x6; store the full symmetric inverse.
 template <bool WALL>
 __global__ void __launch_bounds__(kBuildThreads)
 precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ q,
@@ -205,7 +205,7 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
     extern __shared__ __align__(16) double sm[];
     __shared__ double s_n[36];
     __shared__ int s_fail;
-    const int p = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int p = blockIdx.x, tid = threadIdx.x;
     const int tx = tid & 15, ty = tid >> 4;
     const int64_t b0 = offsets[p];
     const int nbp = (int)(offsets[p + 1] - b0);
@@ -259,44 +259,75 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
         return;
     }
 
-    // K_p rows of blob i (real lengths): [I | C_i], C_i = [[0, dz, -dy], [-dz, 0, dx], [dy, -dx, 0]]
-    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
-    auto k_entry = [&](int row, int col) -> double {
-        const int i = row / 3, r = row % 3;
-        if (col < 3) return r == col ? 1.0 : 0.0;
-        const double* ri = pos + 3 * (b0 + i);
-        const double dx = ri[0] - qx, dy = ri[1] - qy, dz = ri[2] - qz;
-        const int c = col - 3;
-        if (r == c) return 0.0;
-        if (r == 0) return c == 1 ? dz : -dy;
-        if (r == 1) return c == 0 ? -dz : dx;
-        return c == 0 ? dy : -dx;
-    };
-    if (warp < 6) {
-        const int c = warp;
-        for (int i = lane; i < m; i += 32) Yb[(size_t)i * 6 + c] = k_entry(i, c);
-        __syncwarp();
-        for (int j = 0; j < m; ++j) {                       // L y = k
-            const double yj = Yb[(size_t)j * 6 + c] / A[(size_t)j * ld + j];
-            __syncwarp();
-            if (lane == 0) Yb[(size_t)j * 6 + c] = yj;
-            for (int i = j + 1 + lane; i < m; i += 32) Yb[(size_t)i * 6 + c] -= A[(size_t)i * ld + j] * yj;
-            __syncwarp();
+    // ---- explicit inverse ("dense matrix inversion (e.g., Cholesky factorization)"):
+    // Z = L^-1 in place (column by column from the right: Z[j+1:, j] = -Z[j+1:, j+1:] L[j+1:, j] / L_jj,
+    // thread i takes row i of the product, the column is first copied to `tmp`), then
+    // M^-1 = Z^T Z in place on the lower triangle (row i from rows k >= i, thread c takes column c).
+    double* const tmp = Yb;
+    for (int j = m - 1; j >= 0; --j) {
+        const double ajj = 1.0 / A[(size_t)j * ld + j];
+        for (int i = j + 1 + tid; i < m; i += kBuildThreads) tmp[i] = A[(size_t)i * ld + j];
+        __syncthreads();
+        for (int i = j + 1 + tid; i < m; i += kBuildThreads) {
+            const double* Ai = A + (size_t)i * ld;
+            double sum = 0.0;
+            for (int k = j + 1; k <= i; ++k) sum += Ai[k] * tmp[k];
+            A[(size_t)i * ld + j] = -ajj * sum;
         }
-        for (int j = m - 1; j >= 0; --j) {                  // L^T x = y
-            const double xj = Yb[(size_t)j * 6 + c] / A[(size_t)j * ld + j];
-            __syncwarp();
-            if (lane == 0) Yb[(size_t)j * 6 + c] = xj;
-            for (int i = lane; i < j; i += 32) Yb[(size_t)i * 6 + c] -= A[(size_t)j * ld + i] * xj;
-            __syncwarp();
+        if (tid == 0) A[(size_t)j * ld + j] = ajj;
+        __syncthreads();
+    }
+    for (int i = 0; i < m; ++i) {
+        for (int c0 = 0; c0 <= i; c0 += kBuildThreads) {    // chunks of columns; column i itself is in the last one
+            const int c = c0 + tid;
+            double sum = 0.0;
+            if (c <= i)
+                for (int k = i; k < m; ++k) sum += A[(size_t)k * ld + i] * A[(size_t)k * ld + c];
+            __syncthreads();                               // every thread has read row i and column i
+            if (c <= i) A[(size_t)i * ld + c] = sum;
+            __syncthreads();
         }
     }
+    // mirror: A[c][i] = A[i][c] so that rows are complete
+    for (int e = tid; e < m * m; e += kBuildThreads) {
+        const int i = e / m, c = e % m;
+        if (c > i) A[(size_t)i * ld + c] = A[(size_t)c * ld + i];
+    }
     __syncthreads();
-    if (tid < 36) {
+
+    // Y = M^-1 K_p.  K_p rows of blob b (real lengths): [I | C_b], C_b = [[0, dz, -dy], [-dz, 0, dx], [dy, -dx, 0]]
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    for (int e = tid; e < m * 6; e += kBuildThreads) {
+        const int i = e / 6, c = e % 6;
+        const double* Ai = A + (size_t)i * ld;
+        double sum = 0.0;
+        if (c < 3) {
+            for (int bb = 0; bb < nbp; ++bb) sum += Ai[3 * bb + c];
+        } else {
+            for (int bb = 0; bb < nbp; ++bb) {
+                const double* rb = pos + 3 * (b0 + bb);
+                const double dx = rb[0] - qx, dy = rb[1] - qy, dz = rb[2] - qz;
+                const double m0 = Ai[3 * bb], m1 = Ai[3 * bb + 1], m2 = Ai[3 * bb + 2];
+                sum += c == 3 ? (m2 * dy - m1 * dz) : c == 4 ? (m0 * dz - m2 * dx) : (m1 * dx - m0 * dy);
+            }
+        }
+        Yg[b0 * 18 + e] = sum;
+    }
+    __syncthreads();
+    if (tid < 36) {                                          // K_p^T Y
         const int r = tid / 6, c = tid % 6;
-        double s = 0.0;
-        for (int i = 0; i < m; ++i) s += k_entry(i, r) * Yb[(size_t)i * 6 + c];
-        s_n[tid] = s;
+        const double* Y = Yg + b0 * 18;
+        double sum = 0.0;
+        for (int bb = 0; bb < nbp; ++bb) {
+            const double y0 = Y[(size_t)(3 * bb) * 6 + c], y1 = Y[(size_t)(3 * bb + 1) * 6 + c], y2 = Y[(size_t)(3 * bb + 2) * 6 + c];
+            if (r < 3) sum += r == 0 ? y0 : r == 1 ? y1 : y2;
+            else {
+                const double* rb = pos + 3 * (b0 + bb);
+                const double dx = rb[0] - qx, dy = rb[1] - qy, dz = rb[2] - qz;
+                sum += r == 3 ? (dy * y2 - dz * y1) : r == 4 ? (dz * y0 - dx * y2) : (dx * y1 - dy * y0);
+            }
+        }
+        s_n[tid] = sum;
     }
     __syncthreads();
     if (tid == 0) {                                          // invert the SPD 6x6 (Gauss-Jordan, no pivoting needed)
@@ -319,59 +350,20 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
             for (int c = 0; c < 6; ++c) Ntg[(size_t)p * 36 + 6 * r + c] = ok ? a[r][6 + c] : 0.0;
         info[p] = ok ? 0 : m + 1;
     }
-    // store: S[i][j] = S[j][i] = L[max][min]; Y rows
-    for (int e = tid; e < m * m; e += kBuildThreads) {
-        const int i = e / m, j = e % m;
-        const int hi = i > j ? i : j, lo = i > j ? j : i;
-        if (in_smem) G[e] = A[(size_t)hi * ld + lo];
-        else if (j > i) G[e] = A[(size_t)hi * ld + lo];      // mirror the lower triangle upwards in place
-    }
     if (in_smem)
-        for (int e = tid; e < m * 6; e += kBuildThreads) Yg[b0 * 18 + e] = Yb[e];
+        for (int e = tid; e < m * m; e += kBuildThreads) G[e] = A[(size_t)(e / m) * ld + e % m];
 }
 
 // ------------------------------------------------------------------ preconditioner apply
 // One warp per body: [lambda; U] = P_p^-1 [x; y] (Eq. (19)):
-//   r = Y^T x (= K^T M^-1 x),  U = -N~ (y + r),  t = M^-1 x by L t' = x, L^T t = t',  lambda = t + Y U.
-// The right-hand side lives in the warp's slice of `out` (each warp touches only its own body's
-// entries); row j of the stored factor holds column j of L to the right of the diagonal and row j of
-// L to its left, so both substitutions read one contiguous row per step.
-constexpr int kApplySmallM = 63;                 // bodies up to 21 blobs: factor staged in shared memory
-constexpr int kApplySmallWarpDoubles = 4096;     // 63 * 63 + 63 <= 4096 doubles = 32 KB per warp
-constexpr int kApplySmallWarps = 2;              // 64 KB per CTA, three CTAs per SM
-
-// t <- (L L^T)^-1 t for one body by one warp; S is the stored factor (leading dimension m).
-__device__ __forceinline__ void warp_substitutions(const double* S, double* t, int m, int lane)
-{
-    // forward: for j = 0..m-1: t_j /= L_jj; t_i -= L_ij t_j (i > j); L_ij = S[j][i]
-    for (int j = 0; j < m; ++j) {
-        const double* row = S + (size_t)j * m;
-        const double tj = t[j] / row[j];
-        __syncwarp();
-        if (lane == 0) t[j] = tj;
-        for (int i = j + 1 + lane; i < m; i += 32) t[i] -= row[i] * tj;
-        __syncwarp();
-    }
-    // backward: for j = m-1..0: t_j /= L_jj; t_i -= L_ji t_j (i < j); L_ji = S[j][i]
-    for (int j = m - 1; j >= 0; --j) {
-        const double* row = S + (size_t)j * m;
-        const double tj = t[j] / row[j];
-        __syncwarp();
-        if (lane == 0) t[j] = tj;
-        for (int i = lane; i < j; i += 32) t[i] -= row[i] * tj;
-        __syncwarp();
-    }
-}
-
-// SMALL = true: handles the bodies with 3*blobs <= kApplySmallM -- the warp first copies the whole
-// factor (<= 31 KB) and the right-hand side into its slice of shared memory, so the 2m dependent
-// substitution steps run at shared-memory latency; larger bodies are skipped.  SMALL = false: the
-// other bodies, factor rows read from L2/HBM, right-hand side in the warp's slice of `out`.
-template <bool SMALL>
+//   r = Y^T x (= K^T M^-1 x),  U = -N~ (y + r),  t = M^-1 x,  lambda = t + Y U.
+// One warp per body.  t = (M^(pp))^-1 x is a dense symmetric matrix-vector product: lane l owns
+// rows l, l+32, ... in chunks of 128 rows and walks the columns j, reading the contiguous row j of
+// the stored inverse (= its column j) -- coalesced, every load independent of the arithmetic, so the
+// kernel streams the inverses at memory speed instead of waiting on 2m dependent substitution steps.
 __global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
                                      double* __restrict__ out, int64_t n_blobs, int64_t n_bodies)
 {
-    extern __shared__ __align__(16) double sm_apply[];
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     const int64_t* hdr = static_cast<const int64_t*>(precond);
@@ -379,25 +371,15 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
     const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
     const int64_t b0 = pv.offsets[p];
     const int m = 3 * (int)(pv.offsets[p + 1] - b0);
-    if ((m <= kApplySmallM) != SMALL) return;
-    const double* S = pv.factors + pv.mat_off[p];
-    const double* Y = pv.Y + b0 * 18;
-    const double* Ntg = pv.Nt;
-    const double* x = in + 3 * b0;
+    const double* __restrict__ S = pv.factors + pv.mat_off[p];
+    const double* __restrict__ Y = pv.Y + b0 * 18;
+    const double* __restrict__ x = in + 3 * b0;
     const double* y = in + 3 * n_blobs + 6 * p;
     double* t = out + 3 * b0;
-    double* ts = t;                      // where the substitutions work
-    if (SMALL) {
-        double* mine = sm_apply + (size_t)(threadIdx.x >> 5) * kApplySmallWarpDoubles;
-        for (int e = lane; e < m * m; e += 32) mine[e] = S[e];
-        S = mine;
-        ts = mine + m * m;
-    }
 
     double r[6] = {0, 0, 0, 0, 0, 0};
     for (int i = lane; i < m; i += 32) {
         const double xi = x[i];
-        ts[i] = xi;
 #pragma unroll
         for (int c = 0; c < 6; ++c) r[c] += Y[(size_t)i * 6 + c] * xi;
     }
@@ -408,16 +390,41 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
     for (int a = 0; a < 6; ++a) {
         double s = 0.0;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) s += Ntg[(size_t)p * 36 + 6 * a + c] * r[c];
+        for (int c = 0; c < 6; ++c) s += pv.Nt[(size_t)p * 36 + 6 * a + c] * r[c];
         U[a] = -s;
     }
-    __syncwarp();
-    warp_substitutions(S, ts, m, lane);
-    for (int i = lane; i < m; i += 32) {
-        double s = ts[i];
+    for (int i0 = 0; i0 < m; i0 += 128) {
+        const int i_a = i0 + lane, i_b = i_a + 32, i_c = i_a + 64, i_d = i_a + 96;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        if (i0 + 128 <= m) {
+#pragma unroll 4
+            for (int j = 0; j < m; ++j) {
+                const double* row = S + (size_t)j * m;
+                const double xj = x[j];
+                a0 += row[i_a] * xj; a1 += row[i_b] * xj; a2 += row[i_c] * xj; a3 += row[i_d] * xj;
+            }
+        } else {
+#pragma unroll 4
+            for (int j = 0; j < m; ++j) {
+                const double* row = S + (size_t)j * m;
+                const double xj = x[j];
+                if (i_a < m) a0 += row[i_a] * xj;
+                if (i_b < m) a1 += row[i_b] * xj;
+                if (i_c < m) a2 += row[i_c] * xj;
+                if (i_d < m) a3 += row[i_d] * xj;
+            }
+        }
+        const int idx[4] = {i_a, i_b, i_c, i_d};
+        const double acc[4] = {a0, a1, a2, a3};
 #pragma unroll
-        for (int c = 0; c < 6; ++c) s += Y[(size_t)i * 6 + c] * U[c];
-        t[i] = s;
+        for (int k = 0; k < 4; ++k) {
+            if (idx[k] < m) {
+                double s = acc[k];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) s += Y[(size_t)idx[k] * 6 + c] * U[c];
+                t[idx[k]] = s;
+            }
+        }
     }
     if (lane < 6) {
         double v = U[0];
@@ -706,12 +713,7 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
 
 rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, cudaStream_t st)
 {
-    // two launches, each warp decides from its body's size which of them serves it (no host state)
-    constexpr int small_threads = 32 * kApplySmallWarps;
-    constexpr int small_smem = kApplySmallWarps * kApplySmallWarpDoubles * 8;
-    RPY_CUDA_TRY(cudaFuncSetAttribute(precond_apply_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, small_smem));
-    precond_apply_kernel<true><<<warp_grid(nb, small_threads), small_threads, small_smem, st>>>(precond, in, out, N, nb);
-    precond_apply_kernel<false><<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
+    precond_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }

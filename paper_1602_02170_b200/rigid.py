@@ -171,7 +171,7 @@ class Precond:
 
 def rpy_rigid_precond_build(b: Bodies, variant: str = "wall", a: float = 1.0, eta: float = 1.0,
                             check: bool = True) -> Precond:
-    """Dense M^(pp), Cholesky, Y, N~ for every body (Eqs. (17)-(19)); `variant` 'wall' or 'free'."""
+    """Dense M^(pp), its inverse via Cholesky, Y, N~ for every body (Eqs. (17)-(19)); `variant` 'wall' or 'free'."""
     lib = _lib()
     need = int(lib.rpy_rigid_precond_bytes(b.n_bodies, _hptr(b.h_offsets)))
     if need == 0:
@@ -212,7 +212,7 @@ def rpy_rigid_precond_apply(pc: Precond, x: torch.Tensor, out: Optional[torch.Te
 
 
 def rpy_rigid_precond_get(pc: Precond, body: int):
-    """(factor [m, m] with L below and L^T above the diagonal, N~_pp [6, 6]) of one body."""
+    """((M^(pp))^-1 [m, m], N~_pp [6, 6]) of one body."""
     b = pc.bodies
     m = 3 * int(b.h_offsets[body + 1] - b.h_offsets[body])
     fac = torch.empty((m, m), dtype=torch.float64, device=pc.buf.device)

@@ -1,6 +1,6 @@
 """Rigid-multiblob layer (include/rpy_rigid.h) on the GPU vs the CPU oracles, through the C ABI.
 
-K, K^T, the per-body dense blocks and their Cholesky factors, N~_pp, the preconditioner solve of
+K, K^T, the per-body dense blocks and their inverses, N~_pp, the preconditioner solve of
 Eq. (19), the saddle operator of Eq. (11) and the GMRES solve are each compared element by element
 with oracle/rigid.py (definitions in numpy float64) and oracle/gmres.py (textbook GMRES).
 Tolerances: direct linear algebra 1e-10 relative (condition numbers of
@@ -69,24 +69,23 @@ def test_KT_is_bit_reproducible_and_handles_many_small_bodies():
 
 
 @pytest.mark.parametrize("variant", ["wall", "free"])
-def test_precond_factors_and_body_mobilities(variant):
-    """Every body: stored factor = Cholesky factor of the oracle's M^(pp) (L below, L^T above the
-    diagonal), N~_pp = oracle's single-body (K^T M^-1 K)^-1.  Bodies of 15 and 42 blobs take the
-    shared-memory path, the 60-blob cylinders the global-memory path."""
+def test_precond_inverses_and_body_mobilities(variant):
+    """Every body: stored matrix = inverse of the oracle's M^(pp) (numpy.linalg.inv; symmetric, and
+    M^(pp) times it is the identity), N~_pp = oracle's single-body (K^T M^-1 K)^-1.  Bodies of 15 and
+    42 blobs take the shared-memory path, the 60-blob cylinders the global-memory path."""
     a, eta = 0.9, 1.3
     pos, b, lam, db = mixed(seed=1)
     pc = rigid.rpy_rigid_precond_build(db, variant, a, eta)
     blocks = origid.body_blocks(OV[variant], pos, b.offsets, a, eta)
     for p in range(b.n_bodies):
-        fac, nt = rigid.rpy_rigid_precond_get(pc, p)
-        fac = fac.cpu().numpy(); nt = nt.cpu().numpy()
-        L = np.linalg.cholesky(blocks[p])
-        assert rel(np.tril(fac), L) < 1e-10, p
-        assert np.array_equal(np.triu(fac, 1), np.tril(fac, -1).T)
+        inv, nt = rigid.rpy_rigid_precond_get(pc, p)
+        inv = inv.cpu().numpy(); nt = nt.cpu().numpy()
+        assert rel(inv, np.linalg.inv(blocks[p])) < 1e-9, p
+        assert np.array_equal(inv, inv.T)
+        assert np.abs(blocks[p] @ inv - np.eye(inv.shape[0])).max() < 1e-10
         s = slice(b.offsets[p], b.offsets[p + 1])
         Np = origid.body_mobility(OV[variant], pos[s], b.q[p:p + 1], np.array([0, s.stop - s.start]), a, eta)
         assert rel(nt, Np) < 1e-9, p
-        assert rel(np.tril(fac) @ np.tril(fac).T, blocks[p]) < 1e-12      # L L^T = M^(pp)
 
 
 @pytest.mark.parametrize("variant", ["wall", "free"])
