@@ -56,6 +56,14 @@ WORK = {
     ("f64", "wall"): (59, 10, 95, 18),
     ("f64", "free"): (17, 10, 24, 18),
 }
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/): (config, prec, variant) -> (bytes, file).  Algorithmic bytes of that
+# launch: 172,032 x 24 B of records read + 16 partial slices x 172,032 x 24 B written/accumulated = 70 MB
+# (mostly L2-resident); the point of the figure is that DRAM traffic is ~1e-3 of what an HBM-bound kernel
+# of this duration would move.
+NCU_TRAFFIC = {
+    (3, "f32", "wall"): (8.368128e6 + 10.961152e6, "profiles/r1b_allpairs_sym_cfg3_wall_f32.md"),
+}
 SM_COUNT = 148
 LANES = {"f32": 128, "f64": 64}
 SM_MAX_GHZ = 1.965
@@ -379,7 +387,9 @@ def run_ours(args):
         lane_peak = SM_COUNT * LANES[prec] * SM_MAX_GHZ * 1e9
         roofline = {
             "bound": "alu", "kernel": "allpairs_sym_kernel" if plan["symmetric"] else "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-            "frac": achieved / peak, "traffic": None,
+            "frac": achieved / peak,
+            "traffic": NCU_TRAFFIC.get((args.config, prec, variant), (None, None))[0] if k == 1 else None,
+            "traffic_source": NCU_TRAFFIC.get((args.config, prec, variant), (None, None))[1] if k == 1 else None,
             "peak_source": f"derived: {SM_COUNT} SM x {LANES[prec]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
             "flop_per_pair": flops, "lane_ops_per_pair": instr,
             "pipe_frac": pairs_launch * instr / (k_ms * 1e-3) / lane_peak,
