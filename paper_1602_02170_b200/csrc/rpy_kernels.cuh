@@ -159,7 +159,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
 
     // targets of this thread: rows row_begin + (blockIdx.x*BLOCK*T + t*BLOCK + tid); rows past
     // the end recompute the last row and are not stored.
-    V xi[T], yi[T], zi[T];
+    V xi[T], yi[T], zi[T], zi2[T];
     int64_t row[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
@@ -169,6 +169,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
         xi[t] = L::bc((double)r[0 * W]);
         yi[t] = L::bc((double)r[1 * W]);
         zi[t] = L::bc((double)r[2 * W]);
+        zi2[t] = L::bc(2.0 * (double)r[2 * W]);
     }
 
     double dacc[IS_F64 ? 1 : T][IS_F64 ? 1 : K][3];
@@ -227,7 +228,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
                 // phase 3 (every pair): wall scalars and the product with lambda_j
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    if constexpr (WALL) wall_coef<L>(zi[t], zj, rxy2[t], f[t], G[t], c[t]);
+                    if constexpr (WALL) wall_coef<L>(zi[t], zi2[t], zj, rxy2[t], f[t], G[t], c[t]);
                     else { c[t].al = f[t]; c[t].be = G[t]; }
 #pragma unroll
                     for (int s = 0; s < K; ++s)
@@ -340,7 +341,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
         bulk_g2s(buf0, gbase + (int64_t)tile_of(0) * TILE_BYTES, TILE_BYTES, &full_bar[0]);
     }
 
-    V xi[T], yi[T], zi[T], li[T][3];
+    V xi[T], yi[T], zi[T], zi2[T], li[T][3];
     int64_t row[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
@@ -349,6 +350,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
         xi[t] = L::bc((double)r[0 * W]);
         yi[t] = L::bc((double)r[1 * W]);
         zi[t] = L::bc((double)r[2 * W]);
+        zi2[t] = L::bc(2.0 * (double)r[2 * W]);
         li[t][0] = L::bc((double)r[3 * W]);
         li[t][1] = L::bc((double)r[4 * W]);
         li[t][2] = L::bc((double)r[5 * W]);
@@ -409,7 +411,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
                 }
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    if constexpr (WALL) wall_coef<L>(zi[t], zj, rxy2[t], f[t], G[t], c[t]);
+                    if constexpr (WALL) wall_coef<L>(zi[t], zi2[t], zj, rxy2[t], f[t], G[t], c[t]);
                     else { c[t].al = f[t]; c[t].be = G[t]; }
                     pair_apply<L, WALL>(c[t], lj0, lj1, lj2, acc[t][0], acc[t][1], acc[t][2]);
                     if constexpr (WALL) { V tmp = c[t].ga; c[t].ga = c[t].ep; c[t].ep = tmp; }   // M^T: xz <-> zx
