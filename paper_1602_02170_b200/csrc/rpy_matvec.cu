@@ -13,7 +13,7 @@
 #define RPY_SYM_MINB_F32 3
 #endif
 #ifndef RPY_SYM_MINB_F64
-#define RPY_SYM_MINB_F64 3
+#define RPY_SYM_MINB_F64 4
 #endif
 
 namespace {
