@@ -20,8 +20,10 @@ pair-RHS products N^2 k / t are in "pair_rhs_gps").
             against 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (fp64: 64 lanes), DESIGN.md
   cpu_baseline  the float64 oracle (oracle/) on this box's host cores, on a bounded row sample
 
-N > 1 (torchrun): target rows are sharded across ranks (each rank: its rows x all sources, no
-collective inside the data path), then one NCCL all-gather of u; strong scaling.
+N > 1 (torchrun): the work is sharded across ranks -- one right-hand side: each rank takes 1/N of the
+unordered tile pairs of the symmetric kernel and one NCCL all-reduce adds the partial u; several
+right-hand sides: each rank takes a slice of target rows and one all-gather collects u.  No
+collective inside the kernels; strong scaling.
 --impl reference: times the oracle (this tier has no reference implementation to install).
 """
 from __future__ import annotations
@@ -220,12 +222,20 @@ def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, ran
     force = torch.from_numpy(wl.force).to(dt).to(dev)
     n, k = wl.n_blobs, wl.n_rhs
     fn = binding.rpy_wall_matvec if variant == "wall" else binding.rpy_free_matvec
-    rows = None if world == 1 else sharding.shard_rows(n, rank, world)
+    fn_shard = binding.rpy_wall_matvec_shard if variant == "wall" else binding.rpy_free_matvec_shard
+    # N > 1: one right-hand side -> work shards of the symmetric kernel + all-reduce (sum) of u;
+    #        several -> row shards of the plain kernel + all-gather of u
+    work_shards = world > 1 and k == 1
+    rows = None if (world == 1 or work_shards) else sharding.shard_rows(n, rank, world)
     ws = torch.empty(binding.rpy_matvec_workspace_bytes(prec, n, k), dtype=torch.uint8, device=dev)
     out = torch.empty((k, n if rows is None else rows[1], 3), dtype=dt, device=dev)
-    gathered = sharding.gather_buffers(n, k, world, dt, dev) if world > 1 else None
+    gathered = sharding.gather_buffers(n, k, world, dt, dev) if (world > 1 and not work_shards) else None
 
     def step():
+        if work_shards:
+            fn_shard(pos, force, rank, world, wl.a, wl.eta, out=out, workspace=ws)
+            sharding.reduce_velocities(out)
+            return
         fn(pos, force, wl.a, wl.eta, out=out, workspace=ws, rows=rows)
         if world > 1:
             sharding.gather_velocities(out, n, buffers=gathered, concatenate=False)
@@ -364,7 +374,7 @@ def run_ours(args):
     clocks = clk.summary()
     ms = res["ms_per_step"]
     value = n * n / (ms * 1e-3) / 1e9
-    plan = binding.rpy_matvec_launch_plan(prec, n, k, n // world if world > 1 else n)
+    plan = binding.rpy_matvec_launch_plan(prec, n, k, n // world if (world > 1 and k > 1) else n)
     instr, flops = work_per_pair(prec, variant, k, plan["symmetric"])
 
     line = None
@@ -374,7 +384,7 @@ def run_ours(args):
             k_ms, pre_ms, fin_ms = time_allpairs_kernel(torch, binding, res, wl, variant, max(3, min(args.steps, 10)), flush)
         else:
             k_ms, pre_ms, fin_ms = ms, 0.0, 0.0
-        pairs_launch = (n // world if world > 1 else n) * n
+        pairs_launch = n * n // world
         achieved = pairs_launch * flops / (k_ms * 1e-3) / 1e12
         peak = peak_tflops(prec)
         # measured FMA-chain rate on this GPU, same run (context for the derived peak)
@@ -415,7 +425,9 @@ def run_ours(args):
             "config": {"workload": wl.name, "config_index": args.config, "n_blobs": n, "n_rhs": k,
                        "variant": variant, "a": wl.a, "eta": wl.eta, "seed": wl.meta.get("seed"),
                        "l2": "flushed between steps (256 MiB write)",
-                       "parallelism": "single GPU" if world == 1 else f"target rows sharded over {world} ranks + all-gather of u",
+                       "parallelism": "single GPU" if world == 1 else (
+                           f"unordered tile pairs of the symmetric kernel sharded over {world} ranks + all-reduce of u" if k == 1
+                           else f"target rows sharded over {world} ranks + all-gather of u"),
                        "launch_plan": plan},
             "pair_rhs_gps": value * k,
             "clocks": clocks, "e2e": e2e, "gpu_launches": 3 * args.steps * (1 if k <= 8 else -(-k // 8)),

@@ -107,6 +107,23 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
                                 double a, double eta,
                                 void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* Work-sharded forms: one of n_shards PARTIAL products whose sum over shard = 0 .. n_shards-1 is
+ * u = M lambda; the unit a multi-GPU caller gives each rank when it wants the symmetric kernel's
+ * halved arithmetic on every GPU (it then adds the partial results with one all-reduce of
+ * 3 n_rhs n_blobs elements).  d_vel [n_rhs][n_blobs][3] is overwritten with the shard's contribution
+ * to EVERY row.  For n_rhs == 1 and n_blobs >= 6,144 a shard is a contiguous range of the tile
+ * distances of the symmetric kernel (all distances cost the same, so shards are balanced); otherwise
+ * it is a contiguous range of target rows of the plain kernel and the other rows are zero.
+ * 0 <= shard < n_shards <= 4096.  Workspace: rpy_matvec_workspace_bytes().                        */
+rpy_status rpy_wall_matvec_shard(rpy_prec prec, int64_t n_blobs, int n_rhs, int shard, int n_shards,
+                                 const void *d_pos, const void *d_force, void *d_vel,
+                                 double a, double eta,
+                                 void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+rpy_status rpy_free_matvec_shard(rpy_prec prec, int64_t n_blobs, int n_rhs, int shard, int n_shards,
+                                 const void *d_pos, const void *d_force, void *d_vel,
+                                 double a, double eta,
+                                 void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Rectangular product: velocities at n_targets points that are not the sources,
  *   u_t = sum_{j < n_sources} M(r_t, r_j) lambda_j,
  * the flow-field evaluation of Appendix B: "the velocity that a freely-moving

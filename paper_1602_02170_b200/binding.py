@@ -46,6 +46,8 @@ SIGNATURES = {
     "rpy_free_matvec": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_wall_matvec_rows": (_int, [_int, _i64, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_free_matvec_rows": (_int, [_int, _i64, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
+    "rpy_wall_matvec_shard": (_int, [_int, _i64, _int, _int, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
+    "rpy_free_matvec_shard": (_int, [_int, _i64, _int, _int, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_matvec_rect_workspace_bytes": (_sz, [_int, _i64, _i64, _int]),
     "rpy_wall_matvec_rect": (_int, [_int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_free_matvec_rect": (_int, [_int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
@@ -218,6 +220,38 @@ def rpy_free_matvec(pos: torch.Tensor, force: torch.Tensor, a: float = 1.0, eta:
                     rows: Optional[tuple] = None) -> torch.Tensor:
     """u = M lambda with the free-space RPY tensor, Eq. (9)."""
     return _matvec("rpy_free_matvec", pos, force, a, eta, out, workspace, rows)
+
+
+def _matvec_shard(fn_name: str, pos, force, shard, n_shards, a, eta, out, workspace):
+    lib = load_library()
+    _require_cuda(pos, "pos")
+    _require_cuda(force, "force")
+    n, k, single = _shape_inputs(pos, force)
+    prec = _prec_of(pos.dtype)
+    oshape = (n, 3) if single else (k, n, 3)
+    if out is None:
+        out = torch.empty(oshape, dtype=pos.dtype, device=pos.device)
+    elif tuple(out.shape) != oshape or out.dtype != pos.dtype or out.device != pos.device or not out.is_contiguous():
+        raise ValueError(f"out must be a contiguous {pos.dtype} tensor of shape {oshape} on {pos.device}")
+    ws, ws_bytes = _workspace(prec, n, k, pos.device, workspace)
+    with torch.cuda.device(pos.device):
+        stream = torch.cuda.current_stream(pos.device).cuda_stream
+        _check(getattr(lib, fn_name)(prec, n, k, int(shard), int(n_shards), pos.data_ptr() or None,
+                                     force.data_ptr() or None, out.data_ptr() or None, float(a), float(eta),
+                                     ws.data_ptr(), ws_bytes, stream))
+    return out
+
+
+def rpy_wall_matvec_shard(pos: torch.Tensor, force: torch.Tensor, shard: int, n_shards: int, a: float = 1.0,
+                          eta: float = 1.0, *, out=None, workspace=None) -> torch.Tensor:
+    """Shard `shard` of `n_shards` of u = M lambda (wall tensor): a partial result for ALL rows; the
+    sum over the shards is the product (multi-GPU: one all-reduce).  Uses the symmetric kernel."""
+    return _matvec_shard("rpy_wall_matvec_shard", pos, force, shard, n_shards, a, eta, out, workspace)
+
+
+def rpy_free_matvec_shard(pos: torch.Tensor, force: torch.Tensor, shard: int, n_shards: int, a: float = 1.0,
+                          eta: float = 1.0, *, out=None, workspace=None) -> torch.Tensor:
+    return _matvec_shard("rpy_free_matvec_shard", pos, force, shard, n_shards, a, eta, out, workspace)
 
 
 def rpy_matvec_rect_workspace_bytes(prec, n_targets: int, n_sources: int, n_rhs: int = 1) -> int:

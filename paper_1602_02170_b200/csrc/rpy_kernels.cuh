@@ -300,7 +300,7 @@ template <> __device__ __forceinline__ double lane_elem<float2>(float2 v, int w)
 template <class L, bool WALL, int T, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial, double* __restrict__ gacc,
-                    int64_t n_blobs, int nt, int d_per_chunk)
+                    int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end)
 {
     using V = typename L::V;
     using S = typename L::S;
@@ -321,9 +321,11 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int I = blockIdx.x;
     const int D = nt / 2;                          // largest tile distance
-    const int d_lo = blockIdx.y * d_per_chunk;
+    // this launch covers the tile distances d_begin .. d_end-1 (all of 0 .. D unless the work is
+    // sharded over several GPUs: every distance costs the same, so a shard is a range of distances)
+    const int d_lo = d_begin + blockIdx.y * d_per_chunk;
     int d_hi = d_lo + d_per_chunk;
-    if (d_hi > D + 1) d_hi = D + 1;
+    if (d_hi > d_end) d_hi = d_end;
     if ((nt & 1) == 0 && d_hi == D + 1 && I >= D && D > 0) d_hi = D;   // distance nt/2: lower half only
     if (nt == 1) d_hi = d_lo == 0 ? 1 : 0;
     const int my_tiles = d_hi - d_lo;

@@ -20,7 +20,7 @@ namespace {
 
 thread_local int g_last_cuda_error = 0;
 
-constexpr int kAbiVersion = 3;
+constexpr int kAbiVersion = 4;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
 constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
 constexpr int kMaxChunks = 64;
@@ -176,19 +176,24 @@ cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typen
 }
 
 // Symmetric path (rpy::allpairs_sym_kernel): one right-hand side, all rows, enough tiles.
-struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; };
+struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_begin; int d_end; };
+struct Shard { int index; int count; };        // {0, 1}: the whole product
 
 inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
 {
     return K == 1 && row_begin == 0 && rows == n && n >= kSymMinBlobs;
 }
 
-SymPlan make_sym_plan(int64_t n)
+SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
 {
     SymPlan p;
     p.n_padded = (n + kSymTile - 1) / kSymTile * kSymTile;
     p.nt = (int)(p.n_padded / kSymTile);
-    int count = p.nt / 2 + 1;                                  // tile distances 0 .. nt/2
+    const int all = p.nt / 2 + 1;                              // tile distances 0 .. nt/2
+    p.d_begin = (int)((int64_t)all * sh.index / sh.count);     // shard = a contiguous range of distances
+    p.d_end = (int)((int64_t)all * (sh.index + 1) / sh.count);
+    int count = p.d_end - p.d_begin;
+    if (count < 1) count = 1;                                  // an empty shard still launches (and writes zeros)
     int64_t want = (kTargetCtas + p.nt - 1) / p.nt;
     if (want > count) want = count;
     if (want < 1) want = 1;
@@ -208,8 +213,8 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
     constexpr int MINB = SymShape<L>::MINB;
     size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
     dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
-    if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk);
-    else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk);
+    if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+    else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
     return cudaGetLastError();
 }
 
@@ -217,7 +222,8 @@ template <class L, int K>
 cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, typename L::S* vel,
                       double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev,
-                      const typename L::S* tpos /* targets of the rectangular product, else nullptr */)
+                      const typename L::S* tpos /* targets of the rectangular product, else nullptr */,
+                      Shard sh, int64_t vel_stride3 /* elements between right-hand sides of vel */)
 {
     using S = typename L::S;
     S* rec = reinterpret_cast<S*>(ws);
@@ -236,7 +242,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     double* partial = reinterpret_cast<double*>(ws + at);
     const bool sym = !tpos && use_symmetric(n, K, row_begin, rows);
     const Plan p = make_plan(prec, n, K, rows);
-    const SymPlan sp = make_sym_plan(n);
+    const SymPlan sp = make_sym_plan(n, sh);
     const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
     {
         int threads = 256;
@@ -272,7 +278,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int64_t blocks = (per_chunk + threads - 1) / threads;
         const double PI = 3.14159265358979323846;
         rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, vel, per_chunk, n_slices,
-                                                                    rows * 3, rows * 3,
+                                                                    rows * 3, vel_stride3,
                                                                     1.0 / (6.0 * PI * eta * a));
         e = cudaGetLastError();
     }
@@ -283,25 +289,26 @@ template <class L>
 cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
                            const void* d_pos, const void* d_force, void* d_vel,
                            double a, double eta, void* ws, cudaStream_t st, void* const* ev,
-                           const void* d_tpos = nullptr)
+                           const void* d_tpos = nullptr, Shard sh = Shard{0, 1}, int64_t vel_stride3 = -1)
 {
     using S = typename L::S;
     cudaError_t ee;
     if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[0]), st)) != cudaSuccess) return ee;
     const S* pos = static_cast<const S*>(d_pos);
     const S* tp = static_cast<const S*>(d_tpos);
+    if (vel_stride3 < 0) vel_stride3 = rows * 3;
     int done = 0;
     while (done < n_rhs) {
         int K = group_k(n_rhs - done);
         const S* force = static_cast<const S*>(d_force) + (int64_t)done * n * 3;
-        S* vel = static_cast<S*>(d_vel) + (int64_t)done * rows * 3;
+        S* vel = static_cast<S*>(d_vel) + (int64_t)done * vel_stride3;
         unsigned char* w = static_cast<unsigned char*>(ws);
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
-            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
-            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
-            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
@@ -331,6 +338,47 @@ rpy_status matvec_rows(bool wall, rpy_prec prec, int64_t n, int n_rhs, int64_t r
     cudaError_t e = prec == RPY_PREC_F64
         ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev)
         : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, row_begin, rows, d_pos, d_force, d_vel, a, eta, ws, st, ev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
+
+// One of n_shards partial products whose SUM over the shards is u = M lambda (a multi-GPU caller adds
+// them with an all-reduce).  With one right-hand side and enough blobs the shard is a range of tile
+// distances of the symmetric kernel (M_ij = M_ji^T): every shard does 1/n_shards of the
+// unordered pairs and produces contributions to ALL rows.  Otherwise the shard is a range of target
+// rows of the plain kernel and the other rows of its output are zero.
+rpy_status matvec_shard(bool wall, rpy_prec prec, int64_t n, int n_rhs, int shard, int n_shards, const void* d_pos,
+                        const void* d_force, void* d_vel, double a, double eta, void* ws, size_t ws_bytes, void* stream)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n < 0 || n > RPY_MAX_BLOBS || n_rhs < 1 || n_shards < 1 || n_shards > 4096 || shard < 0 || shard >= n_shards) return RPY_ERR_ARG;
+    if (!(a > 0.0) || !(eta > 0.0) || !isfinite(a) || !isfinite(eta)) return RPY_ERR_ARG;
+    if (n == 0) return RPY_OK;
+    if (!d_pos || !d_force || !d_vel || !ws) return RPY_ERR_NULL;
+    size_t es = elem_size(prec);
+    size_t pos_b = (size_t)n * 3 * es, force_b = pos_b * (size_t)n_rhs;
+    size_t need = workspace_bytes(prec, n, n_rhs);
+    if (ws_bytes < need || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    if (overlaps(d_vel, force_b, d_pos, pos_b) || overlaps(d_vel, force_b, d_force, force_b) || overlaps(d_vel, force_b, ws, need))
+        return RPY_ERR_ALIAS;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (n_rhs == 1 && use_symmetric(n, 1, 0, n)) {
+        const Shard sh{shard, n_shards};
+        e = prec == RPY_PREC_F64
+            ? run_all_groups<rpy::Lane<double>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh);
+    } else {
+        const int64_t r0 = n * shard / n_shards, r1 = n * (shard + 1) / n_shards;
+        if ((e = cudaMemsetAsync(d_vel, 0, force_b, st)) != cudaSuccess) return cuda_fail(e);
+        if (r1 == r0) return RPY_OK;
+        void* out = static_cast<unsigned char*>(d_vel) + (size_t)r0 * 3 * es;
+        // rows r0..r1-1 by the plain kernel (never the symmetric one: row_begin/rows are not the whole range,
+        // or n is below the symmetric threshold), written in place of the full-length layout
+        e = prec == RPY_PREC_F64
+            ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3);
+    }
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
 }
@@ -455,6 +503,20 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs, int64
     if (n_blobs < 0) return RPY_ERR_ARG;
     return matvec_rows(false, prec, n_blobs, n_rhs, row_begin, row_count, d_pos, d_force, d_vel, a, eta,
                        d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_wall_matvec_shard(rpy_prec prec, int64_t n_blobs, int n_rhs, int shard, int n_shards, const void* d_pos,
+                                 const void* d_force, void* d_vel, double a, double eta, void* d_workspace,
+                                 size_t workspace_bytes_, void* cuda_stream)
+{
+    return matvec_shard(true, prec, n_blobs, n_rhs, shard, n_shards, d_pos, d_force, d_vel, a, eta, d_workspace, workspace_bytes_, cuda_stream);
+}
+
+rpy_status rpy_free_matvec_shard(rpy_prec prec, int64_t n_blobs, int n_rhs, int shard, int n_shards, const void* d_pos,
+                                 const void* d_force, void* d_vel, double a, double eta, void* d_workspace,
+                                 size_t workspace_bytes_, void* cuda_stream)
+{
+    return matvec_shard(false, prec, n_blobs, n_rhs, shard, n_shards, d_pos, d_force, d_vel, a, eta, d_workspace, workspace_bytes_, cuda_stream);
 }
 
 size_t rpy_matvec_rect_workspace_bytes(rpy_prec prec, int64_t n_targets, int64_t n_sources, int n_rhs)

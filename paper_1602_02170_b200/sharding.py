@@ -1,4 +1,16 @@
-"""Row sharding of the mobility matvec across ranks (one process per GPU).
+"""Sharding of the mobility matvec across ranks (one process per GPU).
+
+Two ways to split u = M lambda over G GPUs, both with every rank holding all positions and forces:
+
+* rows (this module's ``shard_rows`` + ``gather_velocities``): rank r computes its slice of target
+  rows against all sources, then one all-gather.  Needs the plain kernel (every ordered pair).
+* work (``rpy_*_matvec_shard`` + ``reduce_velocities``): rank r computes 1/G of the UNORDERED tile
+  pairs with the symmetric kernel (M_ij = M_ji^T) and so contributes to every row;
+  one all-reduce (sum) of the 3 k N partial velocities gives u on every rank.  Per-GPU arithmetic
+  is 33 instead of 56 FP-pipe operations per ordered pair, at the price of 2x the bytes on NVLink
+  (still O(N) against O(N^2 / G) arithmetic).
+
+Row sharding, in detail:
 
 Rows of M are independent ("trivially parallelized"): rank r computes the
 velocities of a contiguous slice of target blobs against ALL source blobs with
@@ -66,3 +78,11 @@ def gather_velocities(local: torch.Tensor, n_blobs: int, group=None,
     if not concatenate:
         return slices
     return torch.cat(slices, dim=1)
+
+
+def reduce_velocities(partial: torch.Tensor, group=None) -> torch.Tensor:
+    """Sum the per-rank PARTIAL velocities of ``rpy_*_matvec_shard`` (full length on every rank) in
+    place with one all-reduce; returns ``partial``, which then holds u on every rank."""
+    import torch.distributed as dist
+    dist.all_reduce(partial, op=dist.ReduceOp.SUM, group=group)
+    return partial

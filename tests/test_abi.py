@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), f"{n} declared in the header but not exported"
     assert set(names) == set(binding.SIGNATURES), "binding and header disagree on the symbol list"
-    assert lib.rpy_abi_version() == 3
+    assert lib.rpy_abi_version() == 4
 
 
 def test_no_torch_or_oracle_in_native_symbols():

@@ -264,3 +264,26 @@ def test_config4_full_size_sampled_rows():
 @pytest.mark.parametrize("variant", ["wall", "free"])
 def test_config5_full_size_sampled_rows(variant):
     _full_size(5, "f32", variant, 64)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("variant", ["wall", "free"])
+@pytest.mark.parametrize("n_bodies,n_shards,k", [(600, 2, 1), (600, 3, 1), (600, 8, 1), (430, 40, 1), (40, 3, 1), (600, 2, 3)])
+def test_work_shards_sum_to_the_full_product(prec, variant, n_bodies, n_shards, k):
+    """rpy_*_matvec_shard: the partial results of all shards (computed one after the other on this
+    GPU -- on a multi-GPU job each rank computes one and an all-reduce adds them) sum to u.
+    9,000 blobs: symmetric kernel, shards = ranges of tile distances (18 distances: 40 shards leaves
+    some empty); 600 blobs or k = 3: plain kernel, shards = ranges of rows."""
+    w = workloads.config2(seed=4, n_bodies=n_bodies, k=k)
+    pos_b = w.pos.astype(NP[prec]); lam_b = w.force.astype(NP[prec])
+    pos = torch.from_numpy(pos_b).cuda(); lam = torch.from_numpy(lam_b).cuda()
+    fn = binding.rpy_wall_matvec_shard if variant == "wall" else binding.rpy_free_matvec_shard
+    total = torch.zeros((k, w.n_blobs, 3), dtype=torch.float64, device="cuda")
+    for s in range(n_shards):
+        part = fn(pos, lam, s, n_shards)
+        assert part.shape == (k, w.n_blobs, 3)
+        total += part.double()
+    ref = oracle.matvec(ORACLE_VARIANT[variant], pos_b.astype(np.float64), lam_b.astype(np.float64))
+    check(total.cpu().numpy(), ref, prec, f"shards n={w.n_blobs} G={n_shards} {variant}")
+    one = fn(pos, lam, 0, 1)                          # a single shard is the whole product
+    check(one.cpu().numpy().astype(np.float64), ref, prec, "single shard")

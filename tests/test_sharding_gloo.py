@@ -82,3 +82,34 @@ def test_two_rank_gloo_row_sharding_matches_unsharded(tmp_path, n, k):
         assert got.shape == ref.shape == (k, n, 3)
         # rows are independent and the oracle sums each row in a fixed order: bit-identical
         assert np.array_equal(got, ref)
+
+
+def _reduce_worker(rank, world, port, n, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    os.environ["OMP_NUM_THREADS"] = "2"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        w = workloads.config1(seed=5, n=n, k=1)
+        # stand-in for rpy_wall_matvec_shard: a partial product for ALL rows (here: the contribution of
+        # this rank's slice of the sources), full length on every rank
+        lo, cnt = sharding.shard_rows(n, rank, world)
+        lam = np.zeros_like(w.force); lam[:, lo:lo + cnt] = w.force[:, lo:lo + cnt]
+        part = torch.from_numpy(oracle.matvec(oracle.WALL, w.pos, lam, w.a, w.eta))
+        full = sharding.reduce_velocities(part)
+        assert full is part
+        np.save(os.path.join(out_dir, f"red_{rank}.npy"), full.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_work_sharding_all_reduce(tmp_path):
+    import oracle
+    world, n = 2, 157
+    mp.spawn(_reduce_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    w = workloads.config1(seed=5, n=n, k=1)
+    ref = oracle.matvec(oracle.WALL, w.pos, w.force, w.a, w.eta)
+    a, b = np.load(tmp_path / "red_0.npy"), np.load(tmp_path / "red_1.npy")
+    assert np.array_equal(a, b)                       # every rank ends with the same u
+    assert np.allclose(a, ref, rtol=1e-13, atol=1e-15)
