@@ -111,7 +111,7 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
  * u = M lambda; the unit a multi-GPU caller gives each rank when it wants the symmetric kernel's
  * halved arithmetic on every GPU (it then adds the partial results with one all-reduce of
  * 3 n_rhs n_blobs elements).  d_vel [n_rhs][n_blobs][3] is overwritten with the shard's contribution
- * to EVERY row.  For n_rhs == 1 and n_blobs >= 6,144 a shard is a contiguous range of the tile
+ * to EVERY row.  For n_rhs == 1 and n_blobs >= 3,584 a shard is a contiguous range of the tile
  * distances of the symmetric kernel (all distances cost the same, so shards are balanced); otherwise
  * it is a contiguous range of target rows of the plain kernel and the other rows are zero.
  * 0 <= shard < n_shards <= 4096.  Workspace: rpy_matvec_workspace_bytes().                        */
@@ -203,9 +203,9 @@ rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs
  * Pure host arithmetic (no CUDA call); any output pointer may be NULL.
  *   *symmetric == 0: the plain kernel.  A CTA owns *targets_per_cta target rows and walks one of
  *     *n_source_chunks contiguous chunks of the sources in shared-memory tiles of *tile_sources.
- *   *symmetric == 1: the symmetric kernel (n_rhs == 1, all rows, n_blobs >= 6,144), which uses
+ *   *symmetric == 1: the symmetric kernel (n_rhs == 1, all rows, n_blobs >= 3,584), which uses
  *     M_ij = M_ji^T to build every unordered pair's coefficients once.  Blobs are
- *     cut into tiles of *tile_sources (= *targets_per_cta); a CTA owns one tile I and walks the
+ *     cut into tiles of *tile_sources (= *targets_per_cta: 128 below 50,000 blobs, else 256); a CTA owns one tile I and walks the
  *     tiles (I + d) mod n_tiles for one of *n_source_chunks chunks of the distances d = 0..n_tiles/2.
  *     The transposed half of the sum is accumulated with fp64 atomics, so the result is
  *     reproducible to rounding of the double sums (~1e-16 relative), not bit for bit; the plain

@@ -28,7 +28,10 @@ constexpr int kBlock = 128;
 constexpr int kMaxT = 2;
 constexpr size_t kAlign = 256;
 constexpr int kSymTile = kBlock * 2;       // blobs per tile of the symmetric kernel (T = 2)
-constexpr int64_t kSymMinBlobs = 24 * kSymTile;   // below this the plain kernel is used (too few tile pairs per CTA)
+#ifndef RPY_SYM_MIN_BLOBS
+#define RPY_SYM_MIN_BLOBS 3584
+#endif
+constexpr int64_t kSymMinBlobs = RPY_SYM_MIN_BLOBS;   // below this the plain kernel is used (too few tile pairs to fill the chip)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -176,7 +179,11 @@ cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typen
 }
 
 // Symmetric path (rpy::allpairs_sym_kernel): one right-hand side, all rows, enough tiles.
-struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_begin; int d_end; };
+struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_begin; int d_end; int tile; };
+
+#ifndef RPY_SYM_SMALL_BELOW
+#define RPY_SYM_SMALL_BELOW 50000      // below this many blobs the symmetric kernel runs with 128-blob tiles (measured crossover)
+#endif
 struct Shard { int index; int count; };        // {0, 1}: the whole product
 
 inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
@@ -187,8 +194,11 @@ inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
 SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
 {
     SymPlan p;
-    p.n_padded = (n + kSymTile - 1) / kSymTile * kSymTile;
-    p.nt = (int)(p.n_padded / kSymTile);
+    // Tiles of 256 blobs (128 threads x 2 targets) once there are enough of them to fill the chip several
+    // times over; 128-blob tiles (64 threads x 2) below that: four times as many, four times smaller CTAs.
+    p.tile = n < RPY_SYM_SMALL_BELOW ? kSymTile / 2 : kSymTile;
+    p.n_padded = (n + kSymTile - 1) / kSymTile * kSymTile;       // records are padded to 256 either way
+    p.nt = (int)((n + p.tile - 1) / p.tile);
     const int all = p.nt / 2 + 1;                              // tile distances 0 .. nt/2
     p.d_begin = (int)((int64_t)all * sh.index / sh.count);     // shard = a contiguous range of distances
     p.d_end = (int)((int64_t)all * (sh.index + 1) / sh.count);
@@ -211,10 +221,17 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
                        int64_t n, cudaStream_t st)
 {
     constexpr int MINB = SymShape<L>::MINB;
-    size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
     dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
-    if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
-    else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+    if (p.tile == kSymTile) {
+        size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
+        if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+        else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+    } else {
+        constexpr int B2 = kBlock / 2;
+        size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
+        if (wall) rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+        else      rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+    }
     return cudaGetLastError();
 }
 
@@ -630,9 +647,9 @@ rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int
     const int K = group_k(n_rhs);
     if (use_symmetric(n_blobs, K, 0, row_count) && n_rhs == 1) {
         SymPlan sp = make_sym_plan(n_blobs);
-        if (targets_per_cta) *targets_per_cta = kSymTile;
+        if (targets_per_cta) *targets_per_cta = sp.tile;
         if (n_source_chunks) *n_source_chunks = sp.n_chunks;
-        if (tile_sources) *tile_sources = kSymTile;
+        if (tile_sources) *tile_sources = sp.tile;
         if (n_ctas) *n_ctas = (int64_t)sp.nt * sp.n_chunks;
         if (symmetric) *symmetric = 1;
         return RPY_OK;

@@ -76,8 +76,9 @@ def test_launch_plan_covers_all_sources_and_fits_workspace(prec, n, k):
         es = 4 if prec == F32 else 8
         rec = -(-((3 + 3 * kg) * w * es) // 16) * 16
         if p["symmetric"]:
-            # symmetric kernel: one RHS, all rows, tiles of 256 blobs, chunks of the tile distances 0..nt/2
-            assert k == 1 and rows == n and n >= 24 * 256 and ts == tpc == 256
+            # symmetric kernel: one RHS, all rows, tiles of 128 (n < 50,000) or 256 blobs, chunks of the
+            # tile distances 0..nt/2
+            assert k == 1 and rows == n and n >= 3584 and ts == tpc == (128 if n < 50000 else 256)
             nt = -(-n // ts)
             count = nt // 2 + 1
             assert 1 <= nch <= count

@@ -114,20 +114,40 @@ def test_small_shell_lattice_all_rows(prec):
         check(u, ref, "f32", f"cfg5-small {variant}")
 
 
-# ------------------------------------------------------------------ symmetric kernel (n >= 6,144, k = 1, all rows)
+# ------------------------------------------------------------------ symmetric kernel (n >= 3,584, k = 1, all rows)
 @pytest.mark.parametrize("variant", ["wall", "free"])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("n", [6144, 6145, 6400 + 77, 7 * 1024 + 1])
+@pytest.mark.parametrize("n", [3584, 3585, 6144, 6145, 6400 + 77, 7 * 1024 + 1])
 def test_symmetric_kernel_tile_edges(prec, variant, n):
-    """The path that uses M_ij = M_ji^T: even tile count (24: the half-distance case), odd (25),
-    ragged last tile, 29 tiles; dense enough that overlapping pairs (r < 2a) occur across tiles."""
-    assert binding.rpy_matvec_launch_plan(prec, n, 1, n)["symmetric"]
+    """The path that uses M_ij = M_ji^T, 128-blob tiles (n < 50,000): even tile count (28, 48: the
+    half-distance case), odd (29, 49), ragged last tile; dense enough that overlapping pairs
+    (r < 2a) occur across tiles."""
+    plan = binding.rpy_matvec_launch_plan(prec, n, 1, n)
+    assert plan["symmetric"] and plan["tile_sources"] == 128
+    assert not binding.rpy_matvec_launch_plan(prec, 3583, 1, 3583)["symmetric"]
     rng = np.random.default_rng(300 + n)
     side = 40.0
     pos = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(1.1, 9, n)])
     lam = rng.standard_normal((1, n, 3))
     u, ref = run_case(pos, lam, prec, variant, a=0.9, eta=1.7)
     check(u, ref, prec, f"symmetric n={n} {variant}")
+
+
+@pytest.mark.parametrize("variant", ["wall", "free"])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [50176, 50177, 50000 + 3 * 256 + 19])
+def test_symmetric_kernel_256_blob_tiles_sampled_rows(prec, variant, n):
+    """n >= 50,000: 256-blob tiles -- even tile count (196), odd with a one-blob last tile (197), ragged
+    (199); the oracle computes a seeded sample of rows against all sources."""
+    plan = binding.rpy_matvec_launch_plan(prec, n, 1, n)
+    assert plan["symmetric"] and plan["tile_sources"] == 256
+    rng = np.random.default_rng(500 + n)
+    side = 110.0
+    pos = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(1.1, 9, n)])
+    lam = rng.standard_normal((1, n, 3))
+    rows = np.unique(np.concatenate([workloads.sample_rows(n, 700, seed=n), np.arange(n - 300, n), np.arange(0, 40)]))
+    u, ref = run_case(pos, lam, prec, variant, rows=rows)
+    check(u, ref, prec, f"symmetric-256 n={n} {variant}")
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
