@@ -42,6 +42,7 @@ extern "C" {
 
 #define RPY_RIGID_MAX_BODY_BLOBS 512
 #define RPY_RIGID_MAX_RESTART 128
+#define RPY_RIGID_MAX_BATCH 8
 
 /* Additional status (values continue rpy_status): the Cholesky factorisation of some M^(pp) met a
  * non-positive pivot (a blob overlapping the wall, or coincident blobs). */
@@ -136,6 +137,25 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
                                     double *d_lambda, double *d_U,
                                     double *h_history, int *h_n_iter, double *h_rel_resid,
                                     void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* The same for n_rhs (1..RPY_RIGID_MAX_BATCH) right-hand sides at once -- e.g. the columns of the body
+ * mobility matrix N of Eq. (12), one unit force or torque each.  n_rhs independent GMRES processes
+ * advance in lockstep and share every launch, in particular ONE product call with n_rhs right-hand
+ * sides per iteration (the multi-right-hand-side kernel builds each pair tensor once for all of them:
+ * 46 + 10 n_rhs FP-pipe operations per pair instead of 33 per pair and right-hand side).  The iteration
+ * stops when EVERY right-hand side has reached tol (or at max_iter); a zero right-hand side gives zero.
+ *   d_F [n_rhs][n_bodies][6], d_slip [n_rhs][n_blobs][3] or NULL, d_lambda [n_rhs][n_blobs][3],
+ *   d_U [n_rhs][n_bodies][6];  h_history NULL or [n_rhs][max_iter+1];  h_rel_resid [n_rhs];
+ *   workspace: rpy_rigid_solve_batch_workspace_bytes().                                            */
+size_t rpy_rigid_solve_batch_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart,
+                                             int n_rhs);
+rpy_status rpy_rigid_mobility_solve_batch(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int n_rhs,
+                                          const double *d_pos, const double *d_q, const int64_t *d_offsets,
+                                          const double *d_F, const double *d_slip, double a, double eta,
+                                          const void *d_precond, double tol, int restart, int max_iter,
+                                          double *d_lambda, double *d_U,
+                                          double *h_history, int *h_n_iter, double *h_rel_resid,
+                                          void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
 /* The operator of Eq. (11) alone: out = [M lambda - K U ; -K^T lambda] for a solver vector
  * in = [lambda; U] (tests; residual checks).  d_workspace as for the solve with restart = 1.      */

@@ -7,4 +7,10 @@
 namespace rpy {
 // Records `e` as the calling thread's last CUDA error (rpy_last_cuda_error) and returns RPY_ERR_CUDA.
 rpy_status set_cuda_error(cudaError_t e);
+
+// The device product with explicit element strides between the right-hand sides of force and vel
+// (>= 3 n each): lets the batched solver hand over the lambda parts of its solver vectors in place.
+rpy_status matvec_strided(bool wall, rpy_prec prec, int64_t n, int n_rhs, const void* d_pos, const void* d_force,
+                          int64_t force_stride3, void* d_vel, int64_t vel_stride3, double a, double eta,
+                          void* ws, size_t ws_bytes, cudaStream_t st);
 }  // namespace rpy

@@ -240,7 +240,8 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, typename L::S* vel,
                       double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev,
                       const typename L::S* tpos /* targets of the rectangular product, else nullptr */,
-                      Shard sh, int64_t vel_stride3 /* elements between right-hand sides of vel */)
+                      Shard sh, int64_t vel_stride3 /* elements between right-hand sides of vel */,
+                      int64_t force_stride3 /* the same for force */)
 {
     using S = typename L::S;
     S* rec = reinterpret_cast<S*>(ws);
@@ -265,7 +266,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
         rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, n_padded,
-                                                                      n * 3, 1.0 / a);
+                                                                      force_stride3, 1.0 / a);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -306,7 +307,8 @@ template <class L>
 cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
                            const void* d_pos, const void* d_force, void* d_vel,
                            double a, double eta, void* ws, cudaStream_t st, void* const* ev,
-                           const void* d_tpos = nullptr, Shard sh = Shard{0, 1}, int64_t vel_stride3 = -1)
+                           const void* d_tpos = nullptr, Shard sh = Shard{0, 1}, int64_t vel_stride3 = -1,
+                           int64_t force_stride3 = -1)
 {
     using S = typename L::S;
     cudaError_t ee;
@@ -314,18 +316,19 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
     const S* pos = static_cast<const S*>(d_pos);
     const S* tp = static_cast<const S*>(d_tpos);
     if (vel_stride3 < 0) vel_stride3 = rows * 3;
+    if (force_stride3 < 0) force_stride3 = n * 3;
     int done = 0;
     while (done < n_rhs) {
         int K = group_k(n_rhs - done);
-        const S* force = static_cast<const S*>(d_force) + (int64_t)done * n * 3;
+        const S* force = static_cast<const S*>(d_force) + (int64_t)done * force_stride3;
         S* vel = static_cast<S*>(d_vel) + (int64_t)done * vel_stride3;
         unsigned char* w = static_cast<unsigned char*>(ws);
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
-            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
-            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
-            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
@@ -477,6 +480,21 @@ rpy_status matvec_host(bool wall, rpy_prec prec, int64_t n, int n_rhs, const voi
 
 namespace rpy {
 rpy_status set_cuda_error(cudaError_t e) { return cuda_fail(e); }
+
+rpy_status matvec_strided(bool wall, rpy_prec prec, int64_t n, int n_rhs, const void* d_pos, const void* d_force,
+                          int64_t force_stride3, void* d_vel, int64_t vel_stride3, double a, double eta,
+                          void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
+    if (n < 1 || n > RPY_MAX_BLOBS || n_rhs < 1 || force_stride3 < 3 * n || vel_stride3 < 3 * n) return RPY_ERR_ARG;
+    if (!d_pos || !d_force || !d_vel || !ws) return RPY_ERR_NULL;
+    if (ws_bytes < workspace_bytes(prec, n, n_rhs) || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    cudaError_t e = prec == RPY_PREC_F64
+        ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, vel_stride3, force_stride3)
+        : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, vel_stride3, force_stride3);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return RPY_OK;
+}
 }  // namespace rpy
 
 extern "C" {

@@ -32,11 +32,13 @@ inline rpy_status st_of(int s) { return static_cast<rpy_status>(s); }
 // (K U)_i = u_p + omega_p x (r_i - q_p), Eq. (2).
 __global__ void k_apply_kernel(const double* __restrict__ pos, const double* __restrict__ q,
                                const int64_t* __restrict__ offsets, const double* __restrict__ U,
-                               double alpha, double beta, double* __restrict__ out, int64_t n_bodies)
+                               double alpha, double beta, double* __restrict__ out, int64_t n_bodies,
+                               int64_t u_stride, int64_t out_stride /* between right-hand sides (blockIdx.y) */)
 {
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (p >= n_bodies) return;
+    U += (int64_t)blockIdx.y * u_stride; out += (int64_t)blockIdx.y * out_stride;
     const double ux = U[6 * p + 0], uy = U[6 * p + 1], uz = U[6 * p + 2];
     const double wx = U[6 * p + 3], wy = U[6 * p + 4], wz = U[6 * p + 5];
     const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
@@ -65,11 +67,13 @@ __device__ __forceinline__ double warp_sum(double v)
 // f_p = sum lambda_i, tau_p = sum (r_i - q_p) x lambda_i, Eq. (10).
 __global__ void kt_apply_kernel(const double* __restrict__ pos, const double* __restrict__ q,
                                 const int64_t* __restrict__ offsets, const double* __restrict__ lam,
-                                double alpha, double beta, double* __restrict__ out, int64_t n_bodies)
+                                double alpha, double beta, double* __restrict__ out, int64_t n_bodies,
+                                int64_t lam_stride, int64_t out_stride /* between right-hand sides (blockIdx.y) */)
 {
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (p >= n_bodies) return;
+    lam += (int64_t)blockIdx.y * lam_stride; out += (int64_t)blockIdx.y * out_stride;
     const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
     double s[6] = {0, 0, 0, 0, 0, 0};
     for (int64_t i = offsets[p] + lane; i < offsets[p + 1]; i += 32) {
@@ -362,10 +366,12 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
 // the stored inverse (= its column j) -- coalesced, every load independent of the arithmetic, so the
 // kernel streams the inverses at memory speed instead of waiting on 2m dependent substitution steps.
 __global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
-                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies)
+                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies,
+                                     int64_t vec_stride /* between right-hand sides (blockIdx.y) */)
 {
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
+    in += (int64_t)blockIdx.y * vec_stride; out += (int64_t)blockIdx.y * vec_stride;
     const int64_t* hdr = static_cast<const int64_t*>(precond);
     if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
     const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
@@ -435,11 +441,15 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
 }
 
 // ------------------------------------------------------------------ Krylov vector operations
-// Vectors have n = 3 n_blobs + 6 n_bodies doubles.  A fixed grid of kVecBlocks CTAs cuts [0, n)
-// into equal contiguous chunks; every reduction is two-stage (per-CTA partials, then a fixed-order
-// sum), so the solve is bit-reproducible whenever the matvec is.
+// A solver vector has n = 3 n_blobs + 6 n_bodies doubles.  The solver runs `nrhs` independent GMRES
+// processes in lockstep (one right-hand side each: blockIdx.y = right-hand side in every kernel
+// below); vectors of one right-hand side are `ldv` doubles apart, Krylov vector v of right-hand side
+// r is at V + (v * nrhs + r) * ldv.  A fixed grid of kVecBlocks CTAs cuts [0, n) into equal
+// contiguous chunks; every reduction is two-stage (per-CTA partials, then a fixed-order sum), so the
+// solve is bit-reproducible whenever the matvec is.
 constexpr int kVecBlocks = 296;       // 2 CTAs per SM
 constexpr int kVecThreads = 256;
+constexpr int kScal = 8;              // doubles of scalar state per right-hand side
 
 __device__ __forceinline__ void chunk_of(int64_t n, int64_t& lo, int64_t& hi)
 {
@@ -449,48 +459,52 @@ __device__ __forceinline__ void chunk_of(int64_t n, int64_t& lo, int64_t& hi)
     if (lo > n) lo = n;
 }
 
-// partial[v * gridDim.x + blk] = sum over the CTA's chunk of V[v][i] * w[i], v = 0..nvec-1.
+// partial[(r * pvec + v) * gridDim.x + blk] = sum over the CTA's chunk of V[v][r][i] * w[r][i].
 // Warp w of the CTA takes v = w, w + 8, ...; no CTA barrier.
 __global__ void __launch_bounds__(kVecThreads)
-dots_kernel(const double* __restrict__ V, int64_t ldv, int nvec, const double* __restrict__ w, int64_t n,
-            double* __restrict__ partial)
+dots_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, const double* __restrict__ w, int64_t n,
+            double* __restrict__ partial, int pvec)
 {
+    const int r = blockIdx.y;
     int64_t lo, hi; chunk_of(n, lo, hi);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double* wr = w + (int64_t)r * ldv;
     for (int v = warp; v < nvec; v += kVecThreads / 32) {
-        const double* a = V + (int64_t)v * ldv;
+        const double* a = V + ((int64_t)v * nrhs + r) * ldv;
         double s = 0.0;
-        for (int64_t i = lo + lane; i < hi; i += 32) s += a[i] * w[i];
+        for (int64_t i = lo + lane; i < hi; i += 32) s += a[i] * wr[i];
         s = warp_sum(s);
-        if (lane == 0) partial[(int64_t)v * gridDim.x + blockIdx.x] = s;
+        if (lane == 0) partial[((int64_t)r * pvec + v) * gridDim.x + blockIdx.x] = s;
     }
 }
 
-// h[v] = sum_blk partial[v][blk] (fixed order);  w -= sum_v h[v] V[v];  norm_partial[blk] = |w chunk|^2;
-// CTA 0 also does hcol[v] = (accumulate ? hcol[v] : 0) + h[v].
+// h[v] = sum_blk partial[r][v][blk] (fixed order);  w -= sum_v h[v] V[v];  norm_partial[r][blk] = |w chunk|^2;
+// CTA 0 also does hcol[r][v] = (accumulate ? hcol[r][v] : 0) + h[v].
 __global__ void __launch_bounds__(kVecThreads)
-update_kernel(const double* __restrict__ V, int64_t ldv, int nvec, double* __restrict__ w, int64_t n,
-              const double* __restrict__ partial, double* __restrict__ hcol, int accumulate,
+update_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, double* __restrict__ w, int64_t n,
+              const double* __restrict__ partial, int pvec, double* __restrict__ hcol, int accumulate,
               double* __restrict__ norm_partial)
 {
     __shared__ double h[RPY_RIGID_MAX_RESTART + 1];
     __shared__ double red[kVecThreads / 32];
+    const int r = blockIdx.y;
     for (int v = threadIdx.x >> 5; v < nvec; v += kVecThreads / 32) {      // one warp per dot product
         double s = 0.0;
-        for (int b = threadIdx.x & 31; b < (int)gridDim.x; b += 32) s += partial[(int64_t)v * gridDim.x + b];
+        for (int b = threadIdx.x & 31; b < (int)gridDim.x; b += 32) s += partial[((int64_t)r * pvec + v) * gridDim.x + b];
         s = warp_sum(s);
         if ((threadIdx.x & 31) == 0) {
             h[v] = s;
-            if (blockIdx.x == 0) hcol[v] = (accumulate ? hcol[v] : 0.0) + s;
+            if (blockIdx.x == 0) hcol[(int64_t)r * pvec + v] = (accumulate ? hcol[(int64_t)r * pvec + v] : 0.0) + s;
         }
     }
     __syncthreads();
     int64_t lo, hi; chunk_of(n, lo, hi);
+    double* wr = w + (int64_t)r * ldv;
     double nrm = 0.0;
     for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) {
-        double wi = w[i];
-        for (int v = 0; v < nvec; ++v) wi -= h[v] * V[(int64_t)v * ldv + i];
-        w[i] = wi;
+        double wi = wr[i];
+        for (int v = 0; v < nvec; ++v) wi -= h[v] * V[((int64_t)v * nrhs + r) * ldv + i];
+        wr[i] = wi;
         nrm += wi * wi;
     }
     nrm = warp_sum(nrm);
@@ -499,127 +513,148 @@ update_kernel(const double* __restrict__ V, int64_t ldv, int nvec, double* __res
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int k = 0; k < kVecThreads / 32; ++k) s += red[k];
-        norm_partial[blockIdx.x] = s;
+        norm_partial[(int64_t)r * gridDim.x + blockIdx.x] = s;
     }
 }
 
-// Small state of one GMRES cycle, all on the device (column-major R of restart+1 rows).
+// Small state of one GMRES cycle, all on the device; every array has one slice per right-hand side
+// (slice r of an array with `len` entries per right-hand side starts at r * len).
 struct GmresState {
-    double* R;        // [(restart+1) * restart] rotated Hessenberg (upper triangular after rotation)
+    double* R;        // [(restart+1) * restart] column-major rotated Hessenberg (upper triangular after rotation)
     double* cs;       // [restart]
     double* sn;       // [restart]
     double* g;        // [restart+1] rotated right-hand side
     double* hcol;     // [restart+1] current Hessenberg column (sum of the two Gram-Schmidt passes)
     double* yv;       // [restart]   solution of R y = g
-    double* scal;     // [0] beta or h_{j+1,j}; [1] its reciprocal; [2] |g_{j+1}|; [3] ||b||
+    double* scal;     // [kScal] [0] beta or h_{j+1,j}; [1] its reciprocal; [2] |g_{j+1}|; [3] ||b||
+    int restart;
 };
 
-// Column j of the Hessenberg matrix: hcol[0..j] from Gram-Schmidt, h_{j+1,j} = sqrt(sum norm_partial);
-// earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").
-__global__ void hessenberg_kernel(GmresState st, int j, int ldr, const double* __restrict__ norm_partial, int nblk)
+// Column j of the Hessenberg matrix of right-hand side blockIdx.x: hcol[0..j] from Gram-Schmidt,
+// h_{j+1,j} = sqrt(sum norm_partial); earlier Givens rotations, the new rotation, g update
+// (Saad & Schultz; "GMRES").
+__global__ void hessenberg_kernel(GmresState st, int j, const double* __restrict__ norm_partial, int nblk)
 {
+    const int r = blockIdx.x, m = st.restart, ldr = m + 1;
     double s = 0.0;                                  // one warp: fixed-order strided sums, then shuffles
-    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[b];
+    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
     s = warp_sum(s);
     if (threadIdx.x != 0) return;
+    double* scal = st.scal + (int64_t)r * kScal;
+    double* cs = st.cs + (int64_t)r * m; double* sn = st.sn + (int64_t)r * m;
+    double* g = st.g + (int64_t)r * ldr; const double* hcol = st.hcol + (int64_t)r * ldr;
     const double hn = sqrt(s);
-    st.scal[0] = hn;
-    st.scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
-    double* col = st.R + (size_t)j * ldr;
-    for (int i = 0; i <= j; ++i) col[i] = st.hcol[i];
+    scal[0] = hn;
+    scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
+    double* col = st.R + (int64_t)r * ldr * m + (size_t)j * ldr;
+    for (int i = 0; i <= j; ++i) col[i] = hcol[i];
     col[j + 1] = hn;
     for (int i = 0; i < j; ++i) {
-        const double t = st.cs[i] * col[i] + st.sn[i] * col[i + 1];
-        col[i + 1] = -st.sn[i] * col[i] + st.cs[i] * col[i + 1];
+        const double t = cs[i] * col[i] + sn[i] * col[i + 1];
+        col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
         col[i] = t;
     }
     const double d = hypot(col[j], col[j + 1]);
     const double c = d > 0.0 ? col[j] / d : 1.0, sgn = d > 0.0 ? col[j + 1] / d : 0.0;
-    st.cs[j] = c; st.sn[j] = sgn;
+    cs[j] = c; sn[j] = sgn;
     col[j] = d; col[j + 1] = 0.0;
-    st.g[j + 1] = -sgn * st.g[j];
-    st.g[j] = c * st.g[j];
-    st.scal[2] = fabs(st.g[j + 1]);
+    g[j + 1] = -sgn * g[j];
+    g[j] = c * g[j];
+    scal[2] = fabs(g[j + 1]);
 }
 
 // beta = sqrt(sum partial) at the start of a cycle: g = (beta, 0, ...), scal[0..1] = beta, 1/beta;
 // with set_bnorm, scal[3] = beta (the first cycle starts from x0 = 0, so r0 = b).
-__global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int restart, int set_bnorm)
+__global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int set_bnorm)
 {
+    const int r = blockIdx.x, ldr = st.restart + 1;
     double s = 0.0;
-    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[b];
+    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
     s = warp_sum(s);
     if (threadIdx.x != 0) return;
+    double* scal = st.scal + (int64_t)r * kScal;
+    double* g = st.g + (int64_t)r * ldr;
     const double beta = sqrt(s);
-    st.scal[0] = beta; st.scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; st.scal[2] = beta;
-    if (set_bnorm) st.scal[3] = beta;
-    for (int i = 0; i <= restart; ++i) st.g[i] = i == 0 ? beta : 0.0;
+    scal[0] = beta; scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; scal[2] = beta;
+    if (set_bnorm) scal[3] = beta;
+    for (int i = 0; i < ldr; ++i) g[i] = i == 0 ? beta : 0.0;
 }
 
-// R y = g for the first k columns (back substitution).
-__global__ void solve_y_kernel(GmresState st, int k, int ldr)
+// R y = g for the first k columns (back substitution); a zero pivot (a right-hand side that was
+// already solved exactly, or a zero right-hand side) gives y_i = 0.
+__global__ void solve_y_kernel(GmresState st, int k)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (threadIdx.x != 0) return;
+    const int r = blockIdx.x, m = st.restart, ldr = m + 1;
+    const double* R = st.R + (int64_t)r * ldr * m; const double* g = st.g + (int64_t)r * ldr;
+    double* yv = st.yv + (int64_t)r * m;
     for (int i = k - 1; i >= 0; --i) {
-        double s = st.g[i];
-        for (int c = i + 1; c < k; ++c) s -= st.R[(size_t)c * ldr + i] * st.yv[c];
-        st.yv[i] = s / st.R[(size_t)i * ldr + i];
+        double s = g[i];
+        for (int c = i + 1; c < k; ++c) s -= R[(size_t)c * ldr + i] * yv[c];
+        const double piv = R[(size_t)i * ldr + i];
+        yv[i] = piv != 0.0 ? s / piv : 0.0;
     }
 }
 
-// out[i] = (*scale_ptr) * in[i]
-__global__ void scale_kernel(const double* __restrict__ in, const double* __restrict__ scale_ptr, double* __restrict__ out, int64_t n)
+// out[r][i] = scal[r][which] * in[r][i]
+__global__ void scale_kernel(const double* __restrict__ in, int64_t in_stride, const double* __restrict__ scal, int which,
+                             double* __restrict__ out, int64_t out_stride, int64_t n)
 {
-    const double s = *scale_ptr;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        out[i] = s * in[i];
+    const int r = blockIdx.y;
+    const double s = scal[(int64_t)r * kScal + which];
+    const double* a = in + (int64_t)r * in_stride; double* o = out + (int64_t)r * out_stride;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = s * a[i];
 }
 
-// out[i] = sum_{v<k} y[v] V[v][i]
-__global__ void combine_kernel(const double* __restrict__ V, int64_t ldv, int k, const double* __restrict__ y,
-                               double* __restrict__ out, int64_t n)
+// out[r][i] = sum_{v<k} y[r][v] V[v][r][i]
+__global__ void combine_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int k, const double* __restrict__ y,
+                               int ylen, double* __restrict__ out, int64_t n)
 {
+    const int r = blockIdx.y;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         double s = 0.0;
-        for (int v = 0; v < k; ++v) s += y[v] * V[(int64_t)v * ldv + i];
-        out[i] = s;
+        for (int v = 0; v < k; ++v) s += y[(int64_t)r * ylen + v] * V[((int64_t)v * nrhs + r) * ldv + i];
+        out[(int64_t)r * ldv + i] = s;
     }
 }
 
-// y[i] = alpha * x[i] + beta * y[i]   (beta == 0 overwrites)
-__global__ void axpby_kernel(double alpha, const double* __restrict__ x, double beta, double* __restrict__ y, int64_t n)
+// y[r][i] = alpha * x[r][i] + beta * y[r][i]   (beta == 0 overwrites)
+__global__ void axpby_kernel(double alpha, const double* __restrict__ x, int64_t x_stride, double beta,
+                             double* __restrict__ y, int64_t y_stride, int64_t n)
 {
+    const double* xr = x + (int64_t)blockIdx.y * x_stride; double* yr = y + (int64_t)blockIdx.y * y_stride;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        y[i] = beta == 0.0 ? alpha * x[i] : alpha * x[i] + beta * y[i];
+        yr[i] = beta == 0.0 ? alpha * xr[i] : alpha * xr[i] + beta * yr[i];
 }
 
-// |w chunk|^2 per CTA (the norm of a vector through the same two-stage reduction)
+// |w[r] chunk|^2 per CTA (the norm of a vector through the same two-stage reduction)
 __global__ void __launch_bounds__(kVecThreads)
-norm_partial_kernel(const double* __restrict__ w, int64_t n, double* __restrict__ norm_partial)
+norm_partial_kernel(const double* __restrict__ w, int64_t ldv, int64_t n, double* __restrict__ norm_partial)
 {
     __shared__ double red[kVecThreads / 32];
+    const double* wr = w + (int64_t)blockIdx.y * ldv;
     int64_t lo, hi; chunk_of(n, lo, hi);
     double nrm = 0.0;
-    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) nrm += w[i] * w[i];
+    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) nrm += wr[i] * wr[i];
     nrm = warp_sum(nrm);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = nrm;
     __syncthreads();
     if (threadIdx.x == 0) {
         double s = 0.0;
         for (int k = 0; k < kVecThreads / 32; ++k) s += red[k];
-        norm_partial[blockIdx.x] = s;
+        norm_partial[(int64_t)blockIdx.y * gridDim.x + blockIdx.x] = s;
     }
 }
 
-__global__ void to_float_kernel(const double* __restrict__ in, float* __restrict__ out, int64_t n)
+__global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride, float* __restrict__ out, int64_t out_stride, int64_t n)
 {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        out[i] = (float)in[i];
+    const double* a = in + (int64_t)blockIdx.y * in_stride; float* o = out + (int64_t)blockIdx.y * out_stride;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (float)a[i];
 }
-__global__ void to_double_kernel(const float* __restrict__ in, double* __restrict__ out, int64_t n)
+__global__ void to_double_kernel(const float* __restrict__ in, int64_t in_stride, double* __restrict__ out, int64_t out_stride, int64_t n)
 {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        out[i] = (double)in[i];
+    const float* a = in + (int64_t)blockIdx.y * in_stride; double* o = out + (int64_t)blockIdx.y * out_stride;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (double)a[i];
 }
 
 }  // namespace
@@ -644,76 +679,84 @@ rpy_status check_bodies(int64_t n_blobs, int64_t n_bodies)
 constexpr rpy_prec kPrecMixed = static_cast<rpy_prec>(RPY_PREC_MIXED);
 constexpr double kInnerReduction = 1e-4;     // residual reduction asked of one fp32 cycle (mixed solve)
 
-// Solver workspace, carved from one caller-owned buffer.
+// Solver workspace, carved from one caller-owned buffer (nrhs lockstep right-hand sides).
 struct SolveWs {
-    int64_t n; size_t vec_bytes;
+    int64_t n; size_t vec_bytes; int nrhs;
     double *V, *w, *z, *x, *b;
-    GmresState st; int ldr;
+    GmresState st;
     double *partial, *norm_partial;
     float *pos32, *lam32, *vel32;
     void* mv; size_t mv_bytes;
     size_t total;
 };
 
-SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, void* base)
+size_t mv_bytes_of(rpy_prec prec, int64_t n_blobs, int nrhs)
+{
+    if (prec != kPrecMixed) return rpy_matvec_workspace_bytes(prec, n_blobs, nrhs);
+    const size_t a = rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, nrhs), b = rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, nrhs);
+    return a > b ? a : b;
+}
+
+SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, int nrhs, void* base)
 {
     SolveWs W;
     unsigned char* p = static_cast<unsigned char*>(base);
     size_t at = 0;
     auto take = [&](size_t bytes) { unsigned char* r = p ? p + at : nullptr; at = align_up(at + bytes, kAlign); return r; };
+    const size_t k = (size_t)nrhs;
+    W.nrhs = nrhs;
     W.n = 3 * n_blobs + 6 * n_bodies;
     W.vec_bytes = align_up((size_t)W.n * 8, kAlign);
-    W.V = (double*)take(W.vec_bytes * (size_t)(restart + 1));
-    W.w = (double*)take(W.vec_bytes); W.z = (double*)take(W.vec_bytes);
-    W.x = (double*)take(W.vec_bytes); W.b = (double*)take(W.vec_bytes);
-    W.ldr = restart + 1;
-    W.st.R = (double*)take((size_t)(restart + 1) * restart * 8);
-    W.st.cs = (double*)take((size_t)restart * 8); W.st.sn = (double*)take((size_t)restart * 8);
-    W.st.g = (double*)take((size_t)(restart + 1) * 8); W.st.hcol = (double*)take((size_t)(restart + 1) * 8);
-    W.st.yv = (double*)take((size_t)restart * 8); W.st.scal = (double*)take(8 * 8);
-    W.partial = (double*)take((size_t)kVecBlocks * (restart + 1) * 8);
-    W.norm_partial = (double*)take((size_t)kVecBlocks * 8);
+    W.V = (double*)take(W.vec_bytes * (size_t)(restart + 1) * k);
+    W.w = (double*)take(W.vec_bytes * k); W.z = (double*)take(W.vec_bytes * k);
+    W.x = (double*)take(W.vec_bytes * k); W.b = (double*)take(W.vec_bytes * k);
+    W.st.restart = restart;
+    W.st.R = (double*)take((size_t)(restart + 1) * restart * 8 * k);
+    W.st.cs = (double*)take((size_t)restart * 8 * k); W.st.sn = (double*)take((size_t)restart * 8 * k);
+    W.st.g = (double*)take((size_t)(restart + 1) * 8 * k); W.st.hcol = (double*)take((size_t)(restart + 1) * 8 * k);
+    W.st.yv = (double*)take((size_t)restart * 8 * k); W.st.scal = (double*)take((size_t)kScal * 8 * k);
+    W.partial = (double*)take((size_t)kVecBlocks * (restart + 1) * 8 * k);
+    W.norm_partial = (double*)take((size_t)kVecBlocks * 8 * k);
     if (prec != RPY_PREC_F64) {
-        W.pos32 = (float*)take((size_t)n_blobs * 12); W.lam32 = (float*)take((size_t)n_blobs * 12);
-        W.vel32 = (float*)take((size_t)n_blobs * 12);
+        W.pos32 = (float*)take((size_t)n_blobs * 12); W.lam32 = (float*)take((size_t)n_blobs * 12 * k);
+        W.vel32 = (float*)take((size_t)n_blobs * 12 * k);
     } else { W.pos32 = W.lam32 = W.vel32 = nullptr; }
-    W.mv_bytes = prec == kPrecMixed
-        ? (rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, 1) > rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, 1)
-               ? rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, 1) : rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, 1))
-        : rpy_matvec_workspace_bytes(prec, n_blobs, 1);
+    W.mv_bytes = mv_bytes_of(prec, n_blobs, nrhs);
     W.mv = take(W.mv_bytes);
     W.total = at;
     return W;
 }
 
 inline int64_t vec_stride(const SolveWs& W) { return (int64_t)(W.vec_bytes / 8); }
+inline dim3 vgrid(int nrhs) { return dim3(kVecBlocks, (unsigned)nrhs); }
 
-// out = [M lambda - K U ; -K^T lambda], Eq. (11)'s operator.  pos32 must hold float(pos) for the fp32 product.
+// out[r] = [M lambda_r - K U_r ; -K^T lambda_r] for the nrhs solver vectors in[r] (stride `stride`):
+// Eq. (11)'s operator; ONE product call with n_rhs = nrhs.  pos32 must hold float(pos) for the fp32 product.
 rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* pos, const double* q,
-                  const int64_t* off, double a, double eta, const double* in, double* out, const SolveWs& W,
-                  cudaStream_t st)
+                  const int64_t* off, double a, double eta, const double* in, double* out, int64_t stride,
+                  int nrhs, const SolveWs& W, cudaStream_t st)
 {
     rpy_status s;
     if (prec == RPY_PREC_F64) {
-        s = wall ? rpy_wall_matvec(prec, N, 1, pos, in, out, a, eta, W.mv, W.mv_bytes, st)
-                 : rpy_free_matvec(prec, N, 1, pos, in, out, a, eta, W.mv, W.mv_bytes, st);
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, pos, in, stride, out, stride, a, eta, W.mv, W.mv_bytes, st);
         if (s != RPY_OK) return s;
     } else {
-        to_float_kernel<<<kVecBlocks, 256, 0, st>>>(in, W.lam32, 3 * N);
-        s = wall ? rpy_wall_matvec(prec, N, 1, W.pos32, W.lam32, W.vel32, a, eta, W.mv, W.mv_bytes, st)
-                 : rpy_free_matvec(prec, N, 1, W.pos32, W.lam32, W.vel32, a, eta, W.mv, W.mv_bytes, st);
+        to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N);
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st);
         if (s != RPY_OK) return s;
-        to_double_kernel<<<kVecBlocks, 256, 0, st>>>(W.vel32, out, 3 * N);
+        to_double_kernel<<<vgrid(nrhs), 256, 0, st>>>(W.vel32, 3 * N, out, stride, 3 * N);
     }
-    k_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(pos, q, off, in + 3 * N, -1.0, 1.0, out, nb);
-    kt_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(pos, q, off, in, -1.0, 0.0, out + 3 * N, nb);
+    const dim3 bg(warp_grid(nb, 128), (unsigned)nrhs);
+    k_apply_kernel<<<bg, 128, 0, st>>>(pos, q, off, in + 3 * N, -1.0, 1.0, out, nb, stride, stride);
+    kt_apply_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, -1.0, 0.0, out + 3 * N, nb, stride, stride);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
 
-rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, cudaStream_t st)
+rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, int64_t stride,
+                         int nrhs, cudaStream_t st)
 {
-    precond_apply_kernel<<<warp_grid(nb, 128), 128, 0, st>>>(precond, in, out, N, nb);
+    precond_apply_kernel<<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -732,7 +775,7 @@ rpy_status rpy_rigid_K_apply(int64_t n_blobs, int64_t n_bodies, const double* d_
     if (!d_pos || !d_q || !d_offsets || !d_U || !d_out) return RPY_ERR_NULL;
     if (!isfinite(alpha) || !isfinite(beta)) return RPY_ERR_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    k_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_U, alpha, beta, d_out, n_bodies);
+    k_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_U, alpha, beta, d_out, n_bodies, 0, 0);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -747,7 +790,7 @@ rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double* d
     if (!d_pos || !d_q || !d_offsets || !d_lambda || !d_out) return RPY_ERR_NULL;
     if (!isfinite(alpha) || !isfinite(beta)) return RPY_ERR_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    kt_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_lambda, alpha, beta, d_out, n_bodies);
+    kt_apply_kernel<<<warp_grid(n_bodies, 128), 128, 0, st>>>(d_pos, d_q, d_offsets, d_lambda, alpha, beta, d_out, n_bodies, 0, 0);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -882,7 +925,7 @@ rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void
     const size_t bytes = (size_t)(3 * n_blobs + 6 * n_bodies) * 8;
     const uintptr_t a = (uintptr_t)d_in, b = (uintptr_t)d_out;
     if (a < b + bytes && b < a + bytes) return RPY_ERR_ALIAS;
-    return precond_apply(n_blobs, n_bodies, d_precond, d_in, d_out, static_cast<cudaStream_t>(cuda_stream));
+    return precond_apply(n_blobs, n_bodies, d_precond, d_in, d_out, 0, 1, static_cast<cudaStream_t>(cuda_stream));
 }
 
 rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t* h_offsets, const void* d_precond, int64_t body,
@@ -903,9 +946,15 @@ rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t* h_offsets, con
 
 size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart)
 {
+    return rpy_rigid_solve_batch_workspace_bytes(matvec_prec, n_blobs, n_bodies, restart, 1);
+}
+
+size_t rpy_rigid_solve_batch_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart, int n_rhs)
+{
     if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return 0;
     if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1 || restart < 1 || restart > RPY_RIGID_MAX_RESTART) return 0;
-    return carve(matvec_prec, n_blobs, n_bodies, restart, nullptr).total;
+    if (n_rhs < 1 || n_rhs > RPY_RIGID_MAX_BATCH) return 0;
+    return carve(matvec_prec, n_blobs, n_bodies, restart, n_rhs, nullptr).total;
 }
 
 rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
@@ -918,12 +967,147 @@ rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blob
     if (s != RPY_OK || n_bodies < 1) return RPY_ERR_ARG;
     if (!finite_pos(a) || !finite_pos(eta)) return RPY_ERR_ARG;
     if (!d_pos || !d_q || !d_offsets || !d_in || !d_out || !d_workspace) return RPY_ERR_NULL;
-    SolveWs W = carve(matvec_prec, n_blobs, n_bodies, 1, d_workspace);
+    SolveWs W = carve(matvec_prec, n_blobs, n_bodies, 1, 1, d_workspace);
     if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (matvec_prec == RPY_PREC_F32_ACC64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * n_blobs);
-    return saddle(wall, matvec_prec, n_blobs, n_bodies, d_pos, d_q, d_offsets, a, eta, d_in, d_out, W, st);
+    if (matvec_prec == RPY_PREC_F32_ACC64) to_float_kernel<<<vgrid(1), 256, 0, st>>>(d_pos, 0, W.pos32, 0, 3 * n_blobs);
+    return saddle(wall, matvec_prec, n_blobs, n_bodies, d_pos, d_q, d_offsets, a, eta, d_in, d_out, W.n, 1, W, st);
 }
+
+}  // extern "C"
+
+namespace {
+
+// nrhs GMRES processes in lockstep (one per right-hand side, sharing every kernel launch and ONE
+// product call with n_rhs = nrhs per iteration); nrhs = 1 is the plain solve.
+rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, int nrhs,
+                       const double* d_pos, const double* d_q, const int64_t* d_offsets,
+                       const double* d_F, const double* d_slip, double a, double eta,
+                       const void* d_precond, double tol, int restart, int max_iter,
+                       double* d_lambda, double* d_U, double* h_history, int* h_n_iter, double* h_rel_resid,
+                       void* d_workspace, size_t workspace_bytes, cudaStream_t st)
+{
+    const bool mixed = matvec_prec == kPrecMixed;
+    const rpy_prec inner_prec = mixed ? RPY_PREC_F32_ACC64 : matvec_prec;     // the product inside Arnoldi
+    const rpy_prec outer_prec = mixed ? RPY_PREC_F64 : matvec_prec;           // the product of a restart's residual
+    SolveWs W = carve(matvec_prec, N, nb, restart, nrhs, d_workspace);
+    if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    const int64_t n = W.n, ldv = vec_stride(W);
+    const int pvec = restart + 1;
+    const dim3 vg = vgrid(nrhs);
+
+    int64_t bad = -1;
+    rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
+    if (s != RPY_OK) return s;
+    if (matvec_prec != RPY_PREC_F64) to_float_kernel<<<vgrid(1), 256, 0, st>>>(d_pos, 0, W.pos32, 0, 3 * N);
+
+    // b_r = [slip_r; -F_r], x = 0, r0 = b
+    if (d_slip) axpby_kernel<<<vg, 256, 0, st>>>(1.0, d_slip, 3 * N, 0.0, W.b, ldv, 3 * N);
+    else RPY_CUDA_TRY(cudaMemsetAsync(W.b, 0, W.vec_bytes * (size_t)nrhs, st));
+    axpby_kernel<<<dim3(64, (unsigned)nrhs), 256, 0, st>>>(-1.0, d_F, 6 * nb, 0.0, W.b + 3 * N, ldv, 6 * nb);
+    RPY_CUDA_TRY(cudaMemsetAsync(W.x, 0, W.vec_bytes * (size_t)nrhs, st));
+    norm_partial_kernel<<<vg, kVecThreads, 0, st>>>(W.b, ldv, n, W.norm_partial);
+    cycle_start_kernel<<<nrhs, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, 1);
+    double hs[RPY_RIGID_MAX_BATCH * kScal];
+    double bnorm[RPY_RIGID_MAX_BATCH], beta_cycle[RPY_RIGID_MAX_BATCH], rel[RPY_RIGID_MAX_BATCH];
+    auto read_scal = [&]() -> cudaError_t {
+        cudaError_t e = cudaMemcpyAsync(hs, W.st.scal, sizeof(double) * kScal * nrhs, cudaMemcpyDeviceToHost, st);
+        return e != cudaSuccess ? e : cudaStreamSynchronize(st);
+    };
+    RPY_CUDA_TRY(read_scal());
+    bool any = false;
+    for (int r = 0; r < nrhs; ++r) {
+        bnorm[r] = hs[r * kScal + 3]; beta_cycle[r] = bnorm[r];
+        if (!isfinite(bnorm[r])) return RPY_ERR_ARG;
+        rel[r] = bnorm[r] > 0.0 ? 1.0 : 0.0;
+        any = any || bnorm[r] > 0.0;
+        if (h_history) h_history[(size_t)r * (max_iter + 1)] = rel[r];
+    }
+    int n_iter = 0;
+    const double* rvec = W.b;
+    bool done = !any;
+    auto all_le = [&](const double* v, double t) { for (int r = 0; r < nrhs; ++r) if (v[r] > t) return false; return true; };
+    while (!done) {
+        scale_kernel<<<vg, 256, 0, st>>>(rvec, ldv, W.st.scal, 1, W.V, ldv, n);          // v_0 = r / beta
+        int k = 0;
+        for (int j = 0; j < restart; ++j) {
+            const double* vj = W.V + (int64_t)j * nrhs * ldv;
+            if ((s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st)) != RPY_OK) return s;
+            ++n_iter;
+            // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
+            dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
+            update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 0, W.norm_partial);
+            dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
+            update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 1, W.norm_partial);
+            hessenberg_kernel<<<nrhs, 32, 0, st>>>(W.st, j, W.norm_partial, kVecBlocks);
+            scale_kernel<<<vg, 256, 0, st>>>(W.w, ldv, W.st.scal, 1, W.V + (int64_t)(j + 1) * nrhs * ldv, ldv, n);
+            RPY_CUDA_TRY(read_scal());
+            bool inner_all = true;
+            for (int r = 0; r < nrhs; ++r) {
+                const double res = hs[r * kScal + 2];
+                rel[r] = bnorm[r] > 0.0 ? res / bnorm[r] : 0.0;
+                if (h_history) h_history[(size_t)r * (max_iter + 1) + n_iter] = rel[r];
+                if (rel[r] > tol && res > kInnerReduction * beta_cycle[r]) inner_all = false;
+            }
+            k = j + 1;
+            if (mixed) {
+                // the estimates are residuals of the fp32 operator: end the cycle once every right-hand side has
+                // gained kInnerReduction (or reached tol) and let the fp64 residual below decide
+                if (inner_all || n_iter >= max_iter) break;
+            } else if (all_le(rel, tol) || n_iter >= max_iter) { done = true; break; }
+        }
+        // x += P^-1 (V_k y),  R y = g
+        solve_y_kernel<<<nrhs, 32, 0, st>>>(W.st, k);
+        combine_kernel<<<vg, 256, 0, st>>>(W.V, ldv, nrhs, k, W.st.yv, restart, W.w, n);
+        if ((s = precond_apply(N, nb, d_precond, W.w, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+        axpby_kernel<<<vg, 256, 0, st>>>(1.0, W.z, ldv, 1.0, W.x, ldv, n);
+        if (done) break;
+        // restart: r = b - A x  (mixed solve: with the fp64 product -- the true residual of Eq. (11))
+        if ((s = saddle(wall, outer_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, ldv, nrhs, W, st)) != RPY_OK) return s;
+        axpby_kernel<<<vg, 256, 0, st>>>(1.0, W.b, ldv, -1.0, W.w, ldv, n);
+        norm_partial_kernel<<<vg, kVecThreads, 0, st>>>(W.w, ldv, n, W.norm_partial);
+        cycle_start_kernel<<<nrhs, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, 0);
+        rvec = W.w;
+        if (mixed) {
+            RPY_CUDA_TRY(read_scal());
+            for (int r = 0; r < nrhs; ++r) {
+                beta_cycle[r] = hs[r * kScal + 0];
+                rel[r] = bnorm[r] > 0.0 ? beta_cycle[r] / bnorm[r] : 0.0;
+                if (h_history) h_history[(size_t)r * (max_iter + 1) + n_iter] = rel[r];   // replace the estimate by the true value
+            }
+            if (all_le(rel, tol) || n_iter >= max_iter) done = true;
+        }
+    }
+    axpby_kernel<<<vg, 256, 0, st>>>(1.0, W.x, ldv, 0.0, d_lambda, 3 * N, 3 * N);
+    axpby_kernel<<<dim3(64, (unsigned)nrhs), 256, 0, st>>>(1.0, W.x + 3 * N, ldv, 0.0, d_U, 6 * nb, 6 * nb);
+    RPY_CUDA_TRY(cudaGetLastError());
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));
+    if (h_n_iter) *h_n_iter = n_iter;
+    if (h_rel_resid) for (int r = 0; r < nrhs; ++r) h_rel_resid[r] = rel[r];
+    return RPY_OK;
+}
+
+rpy_status solve_checked(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int n_rhs,
+                         const double* d_pos, const double* d_q, const int64_t* d_offsets,
+                         const double* d_F, const double* d_slip, double a, double eta,
+                         const void* d_precond, double tol, int restart, int max_iter,
+                         double* d_lambda, double* d_U, double* h_history, int* h_n_iter, double* h_rel_resid,
+                         void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return RPY_ERR_ARG;
+    if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1 || n_rhs < 1 || n_rhs > RPY_RIGID_MAX_BATCH) return RPY_ERR_ARG;
+    if (!finite_pos(a) || !finite_pos(eta) || !(tol >= 0.0) || restart < 1 || restart > RPY_RIGID_MAX_RESTART || max_iter < 1)
+        return RPY_ERR_ARG;
+    if (!d_pos || !d_q || !d_offsets || !d_F || !d_precond || !d_lambda || !d_U || !d_workspace) return RPY_ERR_NULL;
+    return solve_batch(wall, matvec_prec, n_blobs, n_bodies, n_rhs, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
+                       tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
+                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+}  // namespace
+
+extern "C" {
 
 rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
                                     const double* d_pos, const double* d_q, const int64_t* d_offsets,
@@ -933,101 +1117,22 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
                                     double* h_history, int* h_n_iter, double* h_rel_resid,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
-    if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return RPY_ERR_ARG;
-    const bool mixed = matvec_prec == kPrecMixed;
-    const rpy_prec inner_prec = mixed ? RPY_PREC_F32_ACC64 : matvec_prec;     // the product inside Arnoldi
-    const rpy_prec outer_prec = mixed ? RPY_PREC_F64 : matvec_prec;           // the product of a restart's residual
-    if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1) return RPY_ERR_ARG;
-    if (!finite_pos(a) || !finite_pos(eta) || !(tol >= 0.0) || restart < 1 || restart > RPY_RIGID_MAX_RESTART || max_iter < 1)
-        return RPY_ERR_ARG;
-    if (!d_pos || !d_q || !d_offsets || !d_F || !d_precond || !d_lambda || !d_U || !d_workspace) return RPY_ERR_NULL;
-    SolveWs W = carve(matvec_prec, n_blobs, n_bodies, restart, d_workspace);
-    if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int64_t N = n_blobs, nb = n_bodies, n = W.n, ldv = vec_stride(W);
+    return solve_checked(wall, matvec_prec, n_blobs, n_bodies, 1, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
+                         tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
+                         workspace_bytes, cuda_stream);
+}
 
-    int64_t bad = -1;
-    rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
-    if (s != RPY_OK) return s;
-    if (matvec_prec != RPY_PREC_F64) to_float_kernel<<<kVecBlocks, 256, 0, st>>>(d_pos, W.pos32, 3 * N);
-
-    // b = [slip; -F], x = 0, r0 = b
-    if (d_slip) RPY_CUDA_TRY(cudaMemcpyAsync(W.b, d_slip, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
-    else RPY_CUDA_TRY(cudaMemsetAsync(W.b, 0, (size_t)N * 24, st));
-    axpby_kernel<<<64, 256, 0, st>>>(-1.0, d_F, 0.0, W.b + 3 * N, 6 * nb);
-    RPY_CUDA_TRY(cudaMemsetAsync(W.x, 0, (size_t)n * 8, st));
-    norm_partial_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.b, n, W.norm_partial);
-    cycle_start_kernel<<<1, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, restart, 1);
-    double bnorm = 0.0;
-    RPY_CUDA_TRY(cudaMemcpyAsync(&bnorm, W.st.scal + 3, 8, cudaMemcpyDeviceToHost, st));
-    RPY_CUDA_TRY(cudaStreamSynchronize(st));
-    if (h_history) h_history[0] = 1.0;
-    int n_iter = 0; double rel = 1.0;
-    if (!(bnorm > 0.0)) {
-        RPY_CUDA_TRY(cudaMemsetAsync(d_lambda, 0, (size_t)N * 24, st));
-        RPY_CUDA_TRY(cudaMemsetAsync(d_U, 0, (size_t)nb * 48, st));
-        RPY_CUDA_TRY(cudaStreamSynchronize(st));
-        if (h_n_iter) *h_n_iter = 0;
-        if (h_rel_resid) *h_rel_resid = 0.0;
-        return isfinite(bnorm) ? RPY_OK : RPY_ERR_ARG;
-    }
-    const double* r = W.b;
-    bool done = false;
-    double beta_cycle = bnorm;                   // norm of the residual the current cycle starts from
-    while (!done) {
-        scale_kernel<<<kVecBlocks, 256, 0, st>>>(r, W.st.scal + 1, W.V, n);          // v_0 = r / beta
-        int k = 0;
-        for (int j = 0; j < restart; ++j) {
-            const double* vj = W.V + (int64_t)j * ldv;
-            if ((s = precond_apply(N, nb, d_precond, vj, W.z, st)) != RPY_OK) return s;
-            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, W, st)) != RPY_OK) return s;
-            ++n_iter;
-            // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
-            dots_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial);
-            update_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial, W.st.hcol, 0, W.norm_partial);
-            dots_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial);
-            update_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.V, ldv, j + 1, W.w, n, W.partial, W.st.hcol, 1, W.norm_partial);
-            hessenberg_kernel<<<1, 32, 0, st>>>(W.st, j, W.ldr, W.norm_partial, kVecBlocks);
-            if (j + 1 <= restart) scale_kernel<<<kVecBlocks, 256, 0, st>>>(W.w, W.st.scal + 1, W.V + (int64_t)(j + 1) * ldv, n);
-            double res = 0.0;
-            RPY_CUDA_TRY(cudaMemcpyAsync(&res, W.st.scal + 2, 8, cudaMemcpyDeviceToHost, st));
-            RPY_CUDA_TRY(cudaStreamSynchronize(st));
-            rel = res / bnorm;
-            if (h_history) h_history[n_iter] = rel;
-            k = j + 1;
-            if (mixed) {
-                // the estimate is the residual of the fp32 operator: end the cycle once it has gained
-                // kInnerReduction (or reached tol) and let the fp64 residual below decide
-                if (!(rel > tol) || !(res > kInnerReduction * beta_cycle) || n_iter >= max_iter) break;
-            } else if (!(rel > tol) || n_iter >= max_iter) { done = true; break; }
-        }
-        // x += P^-1 (V_k y),  R y = g
-        solve_y_kernel<<<1, 32, 0, st>>>(W.st, k, W.ldr);
-        combine_kernel<<<kVecBlocks, 256, 0, st>>>(W.V, ldv, k, W.st.yv, W.w, n);
-        if ((s = precond_apply(N, nb, d_precond, W.w, W.z, st)) != RPY_OK) return s;
-        axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.z, 1.0, W.x, n);
-        if (done) break;
-        // restart: r = b - A x  (mixed solve: with the fp64 product -- the true residual of Eq. (11))
-        if ((s = saddle(wall, outer_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, W, st)) != RPY_OK) return s;
-        axpby_kernel<<<kVecBlocks, 256, 0, st>>>(1.0, W.b, -1.0, W.w, n);
-        norm_partial_kernel<<<kVecBlocks, kVecThreads, 0, st>>>(W.w, n, W.norm_partial);
-        cycle_start_kernel<<<1, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, restart, 0);
-        r = W.w;
-        if (mixed) {
-            RPY_CUDA_TRY(cudaMemcpyAsync(&beta_cycle, W.st.scal, 8, cudaMemcpyDeviceToHost, st));
-            RPY_CUDA_TRY(cudaStreamSynchronize(st));
-            rel = beta_cycle / bnorm;
-            if (h_history) h_history[n_iter] = rel;                 // replace the estimate by the true value
-            if (!(rel > tol) || n_iter >= max_iter) done = true;
-        }
-    }
-    RPY_CUDA_TRY(cudaMemcpyAsync(d_lambda, W.x, (size_t)N * 24, cudaMemcpyDeviceToDevice, st));
-    RPY_CUDA_TRY(cudaMemcpyAsync(d_U, W.x + 3 * N, (size_t)nb * 48, cudaMemcpyDeviceToDevice, st));
-    RPY_CUDA_TRY(cudaGetLastError());
-    RPY_CUDA_TRY(cudaStreamSynchronize(st));
-    if (h_n_iter) *h_n_iter = n_iter;
-    if (h_rel_resid) *h_rel_resid = rel;
-    return RPY_OK;
+rpy_status rpy_rigid_mobility_solve_batch(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int n_rhs,
+                                          const double* d_pos, const double* d_q, const int64_t* d_offsets,
+                                          const double* d_F, const double* d_slip, double a, double eta,
+                                          const void* d_precond, double tol, int restart, int max_iter,
+                                          double* d_lambda, double* d_U,
+                                          double* h_history, int* h_n_iter, double* h_rel_resid,
+                                          void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return solve_checked(wall, matvec_prec, n_blobs, n_bodies, n_rhs, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
+                         tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
+                         workspace_bytes, cuda_stream);
 }
 
 }  // extern "C"

@@ -20,6 +20,7 @@ RPY_ERR_NOT_SPD = 6
 RPY_PREC_MIXED = 2       # solve only: fp32 products inside a cycle, fp64 residual per cycle
 RPY_RIGID_MAX_BODY_BLOBS = 512
 RPY_RIGID_MAX_RESTART = 128
+RPY_RIGID_MAX_BATCH = 8
 
 _vp, _i64, _int, _dbl, _sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
 _i64p, _dblp, _intp = ctypes.POINTER(_i64), ctypes.POINTER(_dbl), ctypes.POINTER(_int)
@@ -36,6 +37,9 @@ SIGNATURES = {
     "rpy_rigid_solve_workspace_bytes": (_sz, [_int, _i64, _i64, _int]),
     "rpy_rigid_mobility_solve": (_int, [_int, _int, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _dbl,
                                         _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp]),
+    "rpy_rigid_solve_batch_workspace_bytes": (_sz, [_int, _i64, _i64, _int, _int]),
+    "rpy_rigid_mobility_solve_batch": (_int, [_int, _int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _dbl,
+                                              _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp]),
     "rpy_rigid_saddle_apply": (_int, [_int, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _sz, _vp]),
 }
 
@@ -270,3 +274,42 @@ def rpy_rigid_mobility_solve(b: Bodies, pc: Precond, F: torch.Tensor, slip: Opti
             _stream(b.pos)))
     return {"lambda": lam, "U": U, "history": list(hist[:n_iter.value + 1]), "n_iter": n_iter.value,
             "rel_resid": rel.value}
+
+
+def rpy_rigid_solve_batch_workspace_bytes(matvec_prec, n_blobs: int, n_bodies: int, restart: int, n_rhs: int) -> int:
+    prec = RPY_PREC_MIXED if matvec_prec in ("mixed", RPY_PREC_MIXED) else _prec_code(matvec_prec)
+    return int(_lib().rpy_rigid_solve_batch_workspace_bytes(prec, int(n_blobs), int(n_bodies), int(restart), int(n_rhs)))
+
+
+def rpy_rigid_mobility_solve_batch(b: Bodies, pc: Precond, F: torch.Tensor, slip: Optional[torch.Tensor] = None,
+                                   variant: str = "wall", a: float = 1.0, eta: float = 1.0, tol: float = 1e-8,
+                                   restart: int = 60, max_iter: int = 200, matvec_prec="f64",
+                                   workspace: Optional[torch.Tensor] = None) -> dict:
+    """Eq. (11) for k = F.shape[0] <= 8 right-hand sides at once (lockstep GMRES sharing one k-right-hand-side
+    product per iteration).  F [k, n_bodies, 6], slip [k, n_blobs, 3] or None.
+    Returns {'lambda' [k,N,3], 'U' [k,nb,6], 'history' [k][n_iter+1], 'n_iter', 'rel_resid' [k]}."""
+    if F.dim() != 3:
+        raise ValueError("F must have shape [k, n_bodies, 6]")
+    k = int(F.shape[0])
+    _f64(F, (k, b.n_bodies, 6), "F")
+    if slip is not None:
+        _f64(slip, (k, b.n_blobs, 3), "slip")
+    prec = RPY_PREC_MIXED if matvec_prec in ("mixed", RPY_PREC_MIXED) else _prec_code(matvec_prec)
+    need = rpy_rigid_solve_batch_workspace_bytes(prec, b.n_blobs, b.n_bodies, restart, k)
+    if need == 0:
+        raise ValueError("invalid sizes, restart length or batch size (1..8)")
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=b.pos.device)
+    lam = torch.empty((k, b.n_blobs, 3), dtype=torch.float64, device=b.pos.device)
+    U = torch.empty((k, b.n_bodies, 6), dtype=torch.float64, device=b.pos.device)
+    hist = (_dbl * (k * (max_iter + 1)))()
+    n_iter, rel = _int(0), (_dbl * k)()
+    with torch.cuda.device(b.pos.device):
+        _check(_lib().rpy_rigid_mobility_solve_batch(
+            1 if variant == "wall" else 0, prec, b.n_blobs, b.n_bodies, k, b.pos.data_ptr(), b.q.data_ptr(),
+            b.offsets.data_ptr(), F.data_ptr(), slip.data_ptr() if slip is not None else None, float(a), float(eta),
+            pc.buf.data_ptr(), float(tol), int(restart), int(max_iter), lam.data_ptr(), U.data_ptr(),
+            hist, ctypes.byref(n_iter), rel, workspace.data_ptr(), int(workspace.numel()), _stream(b.pos)))
+    it = n_iter.value
+    return {"lambda": lam, "U": U, "n_iter": it, "rel_resid": list(rel),
+            "history": [list(hist[r * (max_iter + 1): r * (max_iter + 1) + it + 1]) for r in range(k)]}

@@ -186,7 +186,7 @@ def test_rigid_header_symbols_are_exported_and_bound():
     src = re.sub(r"/\*.*?\*/", "", open(RIGID_HEADER).read(), flags=re.S)
     names = sorted(set(re.findall(r"\b(rpy_rigid_[a-z0-9_A-Z]+)\s*\(", src)))
     lib = rigid._lib()
-    assert len(names) == 11
+    assert len(names) == 13
     for n in names:
         assert hasattr(lib, n), f"{n} declared in rpy_rigid.h but not exported"
     assert set(names) == set(rigid.SIGNATURES)
