@@ -346,6 +346,30 @@ def time_solve(torch, cfg: int, matvec_prec: str, tol: float, restart: int = 60)
             "matvec_share": saddle_ms / (wall_ms / it)}
 
 
+def time_solve_batch(torch, cfg: int, matvec_prec: str, tol: float, k: int = 8, restart: int = 40):
+    """k right-hand sides (random force/torque on every body) solved at once by lockstep GMRES with one
+    k-right-hand-side product per iteration, against k single solves' cost per right-hand side."""
+    from paper_1602_02170_b200 import rigid, workloads
+    wl = workloads.make(cfg, k=1)
+    hb = workloads.bodies_of(wl)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=np.float64)).to(dev)
+    b = rigid.bodies(t(wl.pos), t(hb.q), hb.offsets)
+    F = t(np.random.default_rng(9).standard_normal((k, b.n_bodies, 6)))
+    pc = rigid.rpy_rigid_precond_build(b, "wall", wl.a, wl.eta)
+    ws = torch.empty(rigid.rpy_rigid_solve_batch_workspace_bytes(matvec_prec, b.n_blobs, b.n_bodies, restart, k),
+                     dtype=torch.uint8, device=dev)
+    run = lambda: rigid.rpy_rigid_mobility_solve_batch(b, pc, F, None, "wall", wl.a, wl.eta, tol=tol, restart=restart,
+                                                       matvec_prec=matvec_prec, workspace=ws)
+    run(); torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = run()
+    ms = (time.perf_counter() - t0) * 1e3
+    return {"workload": wl.name, "n_blobs": b.n_blobs, "n_bodies": b.n_bodies, "n_rhs": k, "matvec_prec": matvec_prec,
+            "tol": tol, "restart": restart, "n_iter": r["n_iter"], "rel_resid_max": max(r["rel_resid"]),
+            "solve_ms": ms, "ms_per_iter": ms / max(1, r["n_iter"]), "ms_per_rhs": ms / k}
+
+
 def run_ours(args):
     import torch
     from paper_1602_02170_b200 import binding, workloads
@@ -464,6 +488,14 @@ def run_ours(args):
                 except Exception as e:  # pragma: no cover
                     solves.append({"config": cfg, "matvec_prec": p, "error": repr(e)})
             line["rigid_solve"] = solves
+            batch = []
+            for cfg, p, tol in ((2, "mixed", 1e-8), (3, "mixed", 1e-8)):
+                try:
+                    batch.append(time_solve_batch(torch, cfg, p, tol))
+                    log(f"[bench] batch solve {batch[-1]}")
+                except Exception as e:  # pragma: no cover
+                    batch.append({"config": cfg, "matvec_prec": p, "error": repr(e)})
+            line["rigid_solve_batch"] = batch
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

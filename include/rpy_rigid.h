@@ -1,7 +1,8 @@
 /*
  * rpy_rigid.h -- C ABI of the rigid-multiblob layer around the mobility matvec (SURVEY.md 8(f)
- * rows N1, N2): the kinematic matrix K and its transpose, the block-diagonal preconditioner, and
- * the preconditioned GMRES solve of the mobility problem.  Same library as rpy_matvec.h
+ * rows N1, N2, N4): the kinematic matrix K and its transpose, the block-diagonal preconditioner, the
+ * preconditioned GMRES solve of the mobility problem (one or several right-hand sides), and blob
+ * positions from body poses.  Same library as rpy_matvec.h
  * (librpy_matvec.so), same conventions: plain device / host pointers, no allocation, no state,
  * errors as return codes, sm_100a only, no CPU fallback.
  *
