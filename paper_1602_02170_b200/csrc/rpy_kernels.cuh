@@ -34,12 +34,14 @@ __global__ void prepack_kernel(const typename L::S* __restrict__ pos,
                                const typename L::S* __restrict__ force,   // [K][n][3] of this RHS group
                                typename L::S* __restrict__ rec,
                                int64_t n_blobs, int64_t n_padded, int64_t force_rhs_stride,
-                               double inv_a)
+                               double inv_a, double* __restrict__ zero, int64_t zero_count)
 {
     using S = typename L::S;
     using R = RecLayout<L, K>;
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_padded) return;
+    // the symmetric kernel's atomic accumulator (3 doubles per blob) is cleared here: one launch less
+    for (int64_t e = 3 * j; e < 3 * j + 3 && e < zero_count; ++e) zero[e] = 0.0;
     int64_t g = j / R::W;
     int l = (int)(j % R::W);
     S* r = rec + g * R::LEN;

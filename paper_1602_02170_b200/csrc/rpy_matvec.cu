@@ -262,20 +262,18 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     const Plan p = make_plan(prec, n, K, rows);
     const SymPlan sp = make_sym_plan(n, sh);
     const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
+    cudaError_t e;
+    int n_slices = p.n_chunks;
+    // slice n_chunks of `partial` receives the symmetric kernel's transposed half through fp64 atomics
+    double* gacc = sym ? partial + (int64_t)sp.n_chunks * n * 3 : nullptr;
     {
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
         rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, n_padded,
-                                                                      force_stride3, 1.0 / a);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
+                                                                      force_stride3, 1.0 / a, gacc, sym ? n * 3 : 0);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
-    cudaError_t e;
-    int n_slices = p.n_chunks;
     if (sym) {
-        // slice n_chunks of `partial` receives the transposed half through fp64 atomics
-        double* gacc = partial + (int64_t)sp.n_chunks * n * 3;
-        if ((e = cudaMemsetAsync(gacc, 0, (size_t)n * 3 * sizeof(double), st)) != cudaSuccess) return e;
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
         if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, partial, gacc, n, st);
         else e = cudaErrorInvalidValue;
