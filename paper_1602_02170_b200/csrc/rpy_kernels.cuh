@@ -463,7 +463,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------- finalise
-// vel[s][row][c] = scale * sum_{chunk} partial[chunk][s][row][c], chunks added in index order
+// vel[s][row][c] = scale * sum_{chunk} partial[chunk][s][row][c], chunks added in a fixed order
 // (deterministic), one thread per output element.
 template <class S>
 __global__ void finalise_kernel(const double* __restrict__ partial, S* __restrict__ vel,
@@ -472,8 +472,18 @@ __global__ void finalise_kernel(const double* __restrict__ partial, S* __restric
 {
     int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= per_chunk) return;
-    double sum = 0.0;
-    for (int c = 0; c < n_chunks; ++c) sum += partial[(int64_t)c * per_chunk + e];
+    // four interleaved running sums (fixed assignment chunk -> sum, fixed final order): the loads of
+    // different chunks do not wait on one another
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int c = 0;
+    for (; c + 4 <= n_chunks; c += 4) {
+        s0 += partial[(int64_t)c * per_chunk + e];
+        s1 += partial[(int64_t)(c + 1) * per_chunk + e];
+        s2 += partial[(int64_t)(c + 2) * per_chunk + e];
+        s3 += partial[(int64_t)(c + 3) * per_chunk + e];
+    }
+    for (; c < n_chunks; ++c) s0 += partial[(int64_t)c * per_chunk + e];
+    const double sum = (s0 + s1) + (s2 + s3);
     int64_t s = e / row_count3, q = e % row_count3;
     vel[s * vel_rhs_stride + q] = (S)(sum * scale);
 }
