@@ -222,3 +222,34 @@ def test_rigid_host_arithmetic_and_argument_checks():
     assert lib.rpy_rigid_mobility_solve(*args(-1.0, 10, 1 << 30)) == 2
     assert lib.rpy_rigid_mobility_solve(*args(1e-8, 500, 1 << 30)) == 2
     assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, 64)) == 4
+
+
+def test_rigid_and_sharded_bindings_refuse_cpu_tensors():
+    """No CPU fallback anywhere: the rigid layer, the work shards and the rectangular product raise on
+    host tensors (and on a box without CUDA) instead of computing something else."""
+    import torch
+    from paper_1602_02170_b200 import rigid
+    pos = torch.zeros(6, 3, dtype=torch.float64); q = torch.zeros(2, 3, dtype=torch.float64)
+    with pytest.raises((RuntimeError, ValueError)):
+        rigid.bodies(pos, q, [0, 3, 6])
+    with pytest.raises((RuntimeError, ValueError)):
+        rigid.rpy_rigid_blob_positions(pos, q, torch.zeros(2, 4, dtype=torch.float64))
+    lam = torch.zeros(6, 3, dtype=torch.float64)
+    with pytest.raises((RuntimeError, ValueError)):
+        binding.rpy_wall_matvec_shard(pos, lam, 0, 2)
+    with pytest.raises((RuntimeError, ValueError)):
+        binding.rpy_free_matvec_rect(pos, pos, lam)
+    with pytest.raises((RuntimeError, ValueError)):
+        binding.rpy_flow_subdivide(pos, lam, torch.zeros(3, 3, dtype=torch.float64))
+    # host-side argument checks of the sharded / rectangular entry points (no CUDA call is reached)
+    lib = rigid._lib()                      # the same CDLL, with the rigid signatures set
+    one = ctypes.c_void_p(256)
+    assert lib.rpy_wall_matvec_shard(F64, 10, 1, 2, 2, one, one, one, 1.0, 1.0, one, 1 << 20, None) == 2    # shard >= n_shards
+    assert lib.rpy_wall_matvec_shard(F64, 10, 1, 0, 0, one, one, one, 1.0, 1.0, one, 1 << 20, None) == 2
+    assert lib.rpy_free_matvec_shard(F64, 10, 1, 0, 2, one, one, None, 1.0, 1.0, one, 1 << 20, None) == 1
+    assert lib.rpy_wall_matvec_rect(F64, 5, 10, 1, one, one, one, one, 1.0, 1.0, one, 16, None) == 4
+    assert lib.rpy_wall_matvec_rect(F64, -1, 10, 1, one, one, one, one, 1.0, 1.0, one, 16, None) == 2
+    assert binding.rpy_matvec_rect_workspace_bytes(F64, 100, 200, 1) > binding.rpy_matvec_workspace_bytes(F64, 200, 1)
+    assert lib.rpy_flow_subdivide(F64, 10, 1, 0, one, one, one, one, one, None) == 2
+    assert lib.rpy_rigid_solve_batch_workspace_bytes(F64, 1000, 10, 30, 9) == 0
+    assert lib.rpy_rigid_solve_batch_workspace_bytes(F64, 1000, 10, 30, 8) > 8 * 31 * (3000 + 60) * 8
