@@ -296,3 +296,31 @@ def test_body_mobility_matrix_by_a_batch_of_six_unit_loads():
     U2 = r2["U"].cpu().numpy().reshape(8, 12)
     assert rel(U2[:6].T, N2[:, :6]) < 1e-8 and rel(U2[6], N2[:, 6]) < 1e-8 and rel(U2[7], N2[:, 11]) < 1e-8
     assert r2["n_iter"] > 1
+
+
+def test_config3_full_size_mixed_solve_sampled_rows_checked_by_the_oracle():
+    """4,096 shells x 42 blobs = 172,032 blobs (BASELINE.json config 3), mixed-precision solve to 1e-8 in the
+    bench's launch configuration.  The oracle re-evaluates Eq. (10) on a seeded sample of blob rows
+    (each against ALL blobs) and the force/torque balance of every body; the preconditioner's blocks
+    are checked on sampled bodies."""
+    w = workloads.make(3)
+    b = workloads.bodies_of(w)
+    db = rigid.bodies(dev(w.pos), dev(b.q), b.offsets)
+    slip = 0.1 * np.random.default_rng(8).standard_normal(w.pos.shape)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    for p in (0, 2047, 4095):
+        inv, _ = rigid.rpy_rigid_precond_get(pc, p)
+        s = slice(b.offsets[p], b.offsets[p + 1])
+        assert rel(inv.cpu().numpy(), np.linalg.inv(oracle.dense(oracle.WALL, w.pos[s]))) < 1e-9
+    r = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=1e-8, matvec_prec="mixed")
+    assert r["rel_resid"] <= 1e-8 and r["n_iter"] <= 43
+    lam_g = r["lambda"].cpu().numpy(); U_g = r["U"].cpu().numpy()
+    rows = workloads.sample_rows(w.n_blobs, 768, seed=21)
+    top = oracle.matvec(oracle.WALL, w.pos, lam_g, rows=rows) - origid.K_apply(w.pos, b.q, b.offsets, U_g)[rows] - slip[rows]
+    bot = -origid.KT_apply(w.pos, b.q, b.offsets, lam_g) + b.F
+    bn = np.sqrt(np.sum(slip ** 2) + np.sum(b.F ** 2))
+    # the sampled rows carry ~768/172032 of the squared residual: scale the bound accordingly (x4 slack)
+    res_rows = np.sqrt(np.sum(top ** 2)) / bn
+    res_bal = np.sqrt(np.sum(bot ** 2)) / bn
+    print(f"cfg3 mixed solve: {r['n_iter']} iterations, residual {r['rel_resid']:.2e}; oracle: sampled rows {res_rows:.2e}, balance {res_bal:.2e}")
+    assert res_rows <= 4 * 1e-8 * np.sqrt(768 / w.n_blobs) + 1e-10 and res_bal <= 1e-8
