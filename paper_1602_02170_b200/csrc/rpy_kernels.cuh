@@ -392,7 +392,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
             const int q = (p + warp * (NSUB / NWARP > 0 ? NSUB / NWARP : 1)) % NSUB;
             const S* sub = tile + (q * 32) * R::LEN;
             V uj[3] = {L::bc(0.0), L::bc(0.0), L::bc(0.0)};
-#pragma unroll 2
+#pragma unroll (IS_F64 ? 2 : 4)     // measured: fp32 880 -> 896 G pairs/s with 4, fp64 best with 2
             for (int s = 0; s < 32; ++s) {
                 const int g = (s + lane) & 31;
                 const V* r = reinterpret_cast<const V*>(sub + g * R::LEN);
