@@ -144,3 +144,42 @@ def test_blob_positions_from_poses_by_hand_and_by_group_properties():
     assert np.allclose(two, rigid.blob_positions(t, z, q12[None]), atol=1e-14)
     assert np.allclose(np.linalg.norm(two, axis=1), np.linalg.norm(t, axis=1))
     assert np.allclose(rigid.blob_positions(t, c, q1[None]), t @ workloads.quat_to_rot(q1[None])[0].T + c, atol=1e-14)
+
+
+def test_table6_sphere_near_a_wall_through_the_wall_corrected_body_mobility():
+    """Appendix D / Table VI (Fig. 5): the paper's fits of the
+    mobility of its 642-blob sphere at height H above the wall.  The 42-blob shell (a/s = 1/2, R_h and
+    R_tau from Table I) run through the oracle's WALL pair tensor, K and Eq. (12) must reproduce them:
+    a body-level check of the whole wall correction (translation, rotation and their coupling) that
+    no pair-level pin sees.  Tolerances: the fit's own error plus the 42- vs 642-blob resolution."""
+    fits = {}
+    for l in open(os.path.join(GOLDEN, "table6_fits.txt")):
+        if l.strip() and l[0] != "#":
+            t = l.split(); fits[t[0]] = [float(v) for v in t[1:8]]
+
+    def fit(name, x):
+        de, al, f2, f1, f0, d1, d0 = fits[name]
+        return de + (1.0 / x) ** al * (f2 * x * x + f1 * x + f0) / (x * x + d1 * x + d0)
+
+    pos0 = workloads.shell_template(42)
+    d = np.linalg.norm(pos0[:, None] - pos0[None], axis=2)
+    a = 0.5 * d[d > 1e-9].min()
+    off = np.array([0, 42])
+    Nf = rigid.body_mobility(oracle.FREE, pos0, np.zeros((1, 3)), off, a, 1.0)
+    Rh = 1.0 / (SIXPI * np.trace(Nf[:3, :3]) / 3); Rt = (1.0 / (8 * np.pi * np.trace(Nf[3:, 3:]) / 3)) ** (1 / 3)
+    assert Rh == pytest.approx(1.1220, abs=2e-4) and Rt == pytest.approx(1.1019, abs=2e-4)       # Table I
+    for x in (1.5, 2.0, 3.0, 5.0, 8.0):
+        H = x * Rh
+        N = rigid.body_mobility(oracle.WALL, pos0 + [0, 0, H], np.array([[0, 0, H]]), off, a, 1.0)
+        tt = 0.5 * (N[0, 0] + N[1, 1]) * SIXPI * Rh
+        rr_par = 0.5 * (N[3, 3] + N[4, 4]) * 8 * np.pi * Rt ** 3
+        rr_perp = N[5, 5] * 8 * np.pi * Rt ** 3
+        rt = 0.5 * (N[0, 4] - N[1, 3]) * SIXPI * Rh ** 2          # u_x from tau_y = -(u_y from tau_x)
+        assert tt == pytest.approx(fit("tt_par", x), rel=8e-3)
+        assert rr_par == pytest.approx(fit("rr_par", x), rel=8e-3)
+        assert rr_perp == pytest.approx(fit("rr_perp", x), rel=3e-3)
+        assert N[0, 4] == pytest.approx(-N[1, 3], rel=2e-2)        # isotropy in the wall plane, up to the shell's own
+                                                                   # anisotropy (the paper averages over orientations)
+        if x <= 5.0:
+            assert rt == pytest.approx(fit("rt_par", x), rel=5e-2)
+        assert N[2, 2] < 0.5 * (N[0, 0] + N[1, 1])                # perpendicular motion is hindered more (Fig. 5)
