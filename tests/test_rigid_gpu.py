@@ -324,3 +324,29 @@ def test_config3_full_size_mixed_solve_sampled_rows_checked_by_the_oracle():
     res_bal = np.sqrt(np.sum(bot ** 2)) / bn
     print(f"cfg3 mixed solve: {r['n_iter']} iterations, residual {r['rel_resid']:.2e}; oracle: sampled rows {res_rows:.2e}, balance {res_bal:.2e}")
     assert res_rows <= 4 * 1e-8 * np.sqrt(768 / w.n_blobs) + 1e-10 and res_bal <= 1e-8
+
+
+def test_table6_sphere_near_a_wall_on_the_gpu():
+    """The paper's printed fit of mu_tt parallel (Table VI) straight from the CUDA path:
+    42-blob shell (a/s = 1/2) at H = 2 and 3 R_h, six unit loads in one batched solve."""
+    import os
+    fits = {}
+    for l in open(os.path.join(os.path.dirname(__file__), "golden", "table6_fits.txt")):
+        if l.strip() and l[0] != "#":
+            t = l.split(); fits[t[0]] = [float(v) for v in t[1:8]]
+    pos0 = workloads.shell_template(42)
+    d = np.linalg.norm(pos0[:, None] - pos0[None], axis=2)
+    a = 0.5 * d[d > 1e-9].min()
+    Rh, Rt = 1.1220, 1.1019                                   # Table I, 42 blobs, a/s = 1/2
+    F = np.eye(6).reshape(6, 1, 6)
+    for x in (2.0, 3.0):
+        H = x * Rh
+        db = rigid.bodies(dev(pos0 + [0, 0, H]), dev(np.array([[0, 0, H]])), np.array([0, 42]))
+        pc = rigid.rpy_rigid_precond_build(db, "wall", a, 1.0)
+        N = rigid.rpy_rigid_mobility_solve_batch(db, pc, dev(F), None, "wall", a, 1.0, tol=1e-12)["U"].cpu().numpy().reshape(6, 6).T
+        for name, val in (("tt_par", 0.5 * (N[0, 0] + N[1, 1]) * 6 * np.pi * Rh),
+                          ("rr_par", 0.5 * (N[3, 3] + N[4, 4]) * 8 * np.pi * Rt ** 3),
+                          ("rr_perp", N[5, 5] * 8 * np.pi * Rt ** 3)):
+            de, al, f2, f1, f0, d1, d0 = fits[name]
+            fit = de + (1.0 / x) ** al * (f2 * x * x + f1 * x + f0) / (x * x + d1 * x + d0)
+            assert val == pytest.approx(fit, rel=8e-3), (name, x)
