@@ -350,3 +350,21 @@ def test_table6_sphere_near_a_wall_on_the_gpu():
             de, al, f2, f1, f0, d1, d0 = fits[name]
             fit = de + (1.0 / x) ** al * (f2 * x * x + f1 * x + f0) / (x * x + d1 * x + d0)
             assert val == pytest.approx(fit, rel=8e-3), (name, x)
+
+
+def test_table1_effective_radii_on_the_gpu():
+    """Table I (left), straight from the CUDA path: free-space RPY product, K, K^T, the
+    preconditioner and the batched solve give R_h/R_g and R_tau/R_g of the 12- and 42-blob shells."""
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "table1_radii.txt"))
+            if l.strip() and l[0] != "#"]
+    F = np.eye(6).reshape(6, 1, 6)
+    for nb, a_over_s, rh_exp, rt_exp in rows:
+        pos = workloads.shell_template(int(nb))
+        d = np.linalg.norm(pos[:, None] - pos[None], axis=2)
+        a = float(a_over_s) * d[d > 1e-9].min()
+        db = rigid.bodies(dev(pos), dev(np.zeros((1, 3))), np.array([0, int(nb)]))
+        pc = rigid.rpy_rigid_precond_build(db, "free", a, 1.0)
+        N = rigid.rpy_rigid_mobility_solve_batch(db, pc, dev(F), None, "free", a, 1.0, tol=1e-12)["U"].cpu().numpy().reshape(6, 6).T
+        assert 1.0 / (6 * np.pi * np.trace(N[:3, :3]) / 3) == pytest.approx(float(rh_exp), abs=1.5e-4)
+        assert (1.0 / (8 * np.pi * np.trace(N[3:, 3:]) / 3)) ** (1 / 3) == pytest.approx(float(rt_exp), abs=1.5e-4)
