@@ -109,15 +109,17 @@ def config1(seed: int = 0, n: int = 2000, k: int = 1) -> Workload:
                     precisions=("f64",), meta={"seed": seed})
 
 
-def config2(seed: int = 0, n_bodies: int = 1000, k: int = 1) -> Workload:
+def config2(seed: int = 0, n_bodies: int = 1000, k: int = 1, side: float = 400.0) -> Workload:
     """Boomerangs near the wall.  Draw order: quaternions N(0,1)[nb,4] (normalised),
-    centre x ~ U(0,400), y ~ U(0,400), z = |N(0, std 2)| + 2.5, then lambda.
-    The body 'centre' is the corner blob; every blob is then clamped to z >= 1.1."""
+    centre x ~ U(0,side), y ~ U(0,side), z = |N(0, std 2)| + 2.5, then lambda.
+    The body 'centre' is the corner blob; every blob is then clamped to z >= 1.1.
+    side = 400 is BASELINE.json's box; other values keep the number density when n_bodies changes
+    (side = 400 sqrt(n_bodies / 1000): the scaling study of Table III, right)."""
     rng = np.random.default_rng(seed)
     q = rng.standard_normal((n_bodies, 4))
     q /= np.linalg.norm(q, axis=1, keepdims=True)
-    cx = rng.uniform(0.0, 400.0, n_bodies)
-    cy = rng.uniform(0.0, 400.0, n_bodies)
+    cx = rng.uniform(0.0, side, n_bodies)
+    cy = rng.uniform(0.0, side, n_bodies)
     cz = np.abs(rng.normal(0.0, 2.0, n_bodies)) + 2.5
     tmpl = boomerang_template()
     R = quat_to_rot(q)
