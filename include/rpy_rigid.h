@@ -125,6 +125,8 @@ size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, in
  * product M lambda (rpy_wall_matvec / rpy_free_matvec with matvec_prec), K, K^T, classical
  * Gram-Schmidt applied twice, and a Givens update of the small Hessenberg problem -- all on the
  * device; the host reads one double (the residual norm) per iteration, so the call SYNCHRONISES.
+ * That read-back runs on a second stream created (and destroyed) inside the call, while `cuda_stream`
+ * already applies the preconditioner of the next iteration: the only CUDA objects the library creates.
  *   wall        != 0: wall-corrected M in the product (the preconditioner is whatever was built)
  *   d_F         [n_bodies][6] device;  d_slip [n_blobs][3] device or NULL (zero slip)
  *   d_lambda    [n_blobs][3], d_U [n_bodies][6] : device, overwritten

@@ -978,6 +978,20 @@ rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blob
 
 namespace {
 
+// A second stream and an event that live for the duration of one solve: the residual norm travels to
+// the host on the side stream while the main stream already applies the preconditioner of the NEXT
+// iteration, so the host's read-back latency is covered by device work (the speculative application
+// is wasted only in the last iteration).
+struct SideStream {
+    cudaStream_t s2 = nullptr; cudaEvent_t ev = nullptr;
+    cudaError_t init()
+    {
+        cudaError_t e = cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking);
+        return e != cudaSuccess ? e : cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    }
+    ~SideStream() { if (ev) cudaEventDestroy(ev); if (s2) cudaStreamDestroy(s2); }
+};
+
 // nrhs GMRES processes in lockstep (one per right-hand side, sharing every kernel launch and ONE
 // product call with n_rhs = nrhs per iteration); nrhs = 1 is the plain solve.
 rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, int nrhs,
@@ -1014,6 +1028,17 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
         cudaError_t e = cudaMemcpyAsync(hs, W.st.scal, sizeof(double) * kScal * nrhs, cudaMemcpyDeviceToHost, st);
         return e != cudaSuccess ? e : cudaStreamSynchronize(st);
     };
+    SideStream side;
+    RPY_CUDA_TRY(side.init());
+    // the same read-back, but ordered only after what the main stream has done SO FAR: work enqueued on
+    // the main stream between `mark` and `read_marked` overlaps the copy and the host's wait
+    auto mark = [&]() -> cudaError_t { return cudaEventRecord(side.ev, st); };
+    auto read_marked = [&]() -> cudaError_t {
+        cudaError_t e = cudaStreamWaitEvent(side.s2, side.ev, 0);
+        if (e != cudaSuccess) return e;
+        e = cudaMemcpyAsync(hs, W.st.scal, sizeof(double) * kScal * nrhs, cudaMemcpyDeviceToHost, side.s2);
+        return e != cudaSuccess ? e : cudaStreamSynchronize(side.s2);
+    };
     RPY_CUDA_TRY(read_scal());
     bool any = false;
     for (int r = 0; r < nrhs; ++r) {
@@ -1030,9 +1055,11 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
     while (!done) {
         scale_kernel<<<vg, 256, 0, st>>>(rvec, ldv, W.st.scal, 1, W.V, ldv, n);          // v_0 = r / beta
         int k = 0;
+        bool z_ready = false;                    // W.z already holds P^-1 v_j (applied speculatively)
         for (int j = 0; j < restart; ++j) {
             const double* vj = W.V + (int64_t)j * nrhs * ldv;
-            if ((s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+            if (!z_ready && (s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+            z_ready = false;
             if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st)) != RPY_OK) return s;
             ++n_iter;
             // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
@@ -1042,7 +1069,12 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
             update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 1, W.norm_partial);
             hessenberg_kernel<<<nrhs, 32, 0, st>>>(W.st, j, W.norm_partial, kVecBlocks);
             scale_kernel<<<vg, 256, 0, st>>>(W.w, ldv, W.st.scal, 1, W.V + (int64_t)(j + 1) * nrhs * ldv, ldv, n);
-            RPY_CUDA_TRY(read_scal());
+            RPY_CUDA_TRY(mark());
+            if (j + 1 < restart && n_iter < max_iter) {          // speculative: P^-1 v_{j+1} for the next iteration
+                if ((s = precond_apply(N, nb, d_precond, W.V + (int64_t)(j + 1) * nrhs * ldv, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+                z_ready = true;
+            }
+            RPY_CUDA_TRY(read_marked());
             bool inner_all = true;
             for (int r = 0; r < nrhs; ++r) {
                 const double res = hs[r * kScal + 2];
