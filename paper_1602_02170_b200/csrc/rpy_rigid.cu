@@ -4,12 +4,12 @@
 // (PAPER.md:79-84, 154-252).  sm_100a only; no allocation, no state.
 //
 // Kernels:
-//   k_apply / kt_apply        one warp per body; O(N_b)
+//   k_apply / kt_apply / saddle_tail     one warp per body; O(N_b)
 //   precond_build             one CTA per body: dense M^(pp) from the same pair arithmetic as the
 //                             matvec (rpy_math.cuh, double lanes), in-place Cholesky, explicit inverse
 //                             from the factor, Y = M^-1 K, N~ = (K^T Y)^-1
 //   precond_apply             one warp per body: symmetric matrix-vector product + 6x6 work
-//   dots / update / hessenberg / scale / combine      the Krylov vector operations of GMRES
+//   dots / update / normalise (+ Hessenberg) / combine     the Krylov vector operations of GMRES
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -91,6 +91,48 @@ __global__ void kt_apply_kernel(const double* __restrict__ pos, const double* __
 #pragma unroll
         for (int c = 1; c < 6; ++c) if (lane == c) v = s[c];
         out[6 * p + lane] = (beta == 0.0 ? 0.0 : beta * out[6 * p + lane]) + alpha * v;
+    }
+}
+
+// The two O(N) pieces of Eq. (11)'s operator in one pass, one warp per body (blockIdx.y = right-hand side):
+//   out_top[i]  = (vel32 ? double(vel32[i]) : out_top[i]) - (K U)_i        (M lambda is already in place)
+//   out_bot[p]  = -(K^T lambda)_p
+// in = [lambda; U], out = [top; bottom], both with `stride` doubles between right-hand sides.
+__global__ void saddle_tail_kernel(const double* __restrict__ pos, const double* __restrict__ q,
+                                   const int64_t* __restrict__ offsets, const double* __restrict__ in,
+                                   const float* __restrict__ vel32, double* __restrict__ out,
+                                   int64_t n_blobs, int64_t n_bodies, int64_t stride)
+{
+    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (p >= n_bodies) return;
+    in += (int64_t)blockIdx.y * stride; out += (int64_t)blockIdx.y * stride;
+    if (vel32) vel32 += (int64_t)blockIdx.y * 3 * n_blobs;
+    const double* U = in + 3 * n_blobs + 6 * p;
+    const double ux = U[0], uy = U[1], uz = U[2], wx = U[3], wy = U[4], wz = U[5];
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int64_t i = offsets[p] + lane; i < offsets[p + 1]; i += 32) {
+        const double dx = pos[3 * i + 0] - qx, dy = pos[3 * i + 1] - qy, dz = pos[3 * i + 2] - qz;
+        const double m0 = vel32 ? (double)vel32[3 * i + 0] : out[3 * i + 0];
+        const double m1 = vel32 ? (double)vel32[3 * i + 1] : out[3 * i + 1];
+        const double m2 = vel32 ? (double)vel32[3 * i + 2] : out[3 * i + 2];
+        out[3 * i + 0] = m0 - (ux + (wy * dz - wz * dy));
+        out[3 * i + 1] = m1 - (uy + (wz * dx - wx * dz));
+        out[3 * i + 2] = m2 - (uz + (wx * dy - wy * dx));
+        const double lx = in[3 * i + 0], ly = in[3 * i + 1], lz = in[3 * i + 2];
+        s[0] += lx; s[1] += ly; s[2] += lz;
+        s[3] += dy * lz - dz * ly;
+        s[4] += dz * lx - dx * lz;
+        s[5] += dx * ly - dy * lx;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) s[c] = warp_sum(s[c]);
+    if (lane < 6) {
+        double v = s[0];
+#pragma unroll
+        for (int c = 1; c < 6; ++c) if (lane == c) v = s[c];
+        out[3 * n_blobs + 6 * p + lane] = -v;
     }
 }
 
@@ -530,20 +572,14 @@ struct GmresState {
     int restart;
 };
 
-// Column j of the Hessenberg matrix of right-hand side blockIdx.x: hcol[0..j] from Gram-Schmidt,
-// h_{j+1,j} = sqrt(sum norm_partial); earlier Givens rotations, the new rotation, g update
-// (Saad & Schultz; "GMRES").
-__global__ void hessenberg_kernel(GmresState st, int j, const double* __restrict__ norm_partial, int nblk)
+// Column j of the Hessenberg matrix of right-hand side r: hcol[0..j] from Gram-Schmidt, h_{j+1,j} = hn;
+// earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").  One thread.
+__device__ void hessenberg_update(const GmresState& st, int r, int j, double hn)
 {
-    const int r = blockIdx.x, m = st.restart, ldr = m + 1;
-    double s = 0.0;                                  // one warp: fixed-order strided sums, then shuffles
-    for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
-    s = warp_sum(s);
-    if (threadIdx.x != 0) return;
+    const int m = st.restart, ldr = m + 1;
     double* scal = st.scal + (int64_t)r * kScal;
     double* cs = st.cs + (int64_t)r * m; double* sn = st.sn + (int64_t)r * m;
     double* g = st.g + (int64_t)r * ldr; const double* hcol = st.hcol + (int64_t)r * ldr;
-    const double hn = sqrt(s);
     scal[0] = hn;
     scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
     double* col = st.R + (int64_t)r * ldr * m + (size_t)j * ldr;
@@ -561,6 +597,32 @@ __global__ void hessenberg_kernel(GmresState st, int j, const double* __restrict
     g[j + 1] = -sgn * g[j];
     g[j] = c * g[j];
     scal[2] = fabs(g[j + 1]);
+}
+
+// End of Arnoldi step j in ONE launch: every CTA sums the norm partials of its right-hand side
+// (blockIdx.y) in the same fixed order, h_{j+1,j} = sqrt(sum), and writes its chunk of
+// v_{j+1} = w / h_{j+1,j}; CTA 0 of each right-hand side also updates the Hessenberg problem.
+__global__ void __launch_bounds__(kVecThreads)
+normalise_kernel(GmresState st, int j, const double* __restrict__ norm_partial, const double* __restrict__ w,
+                 int64_t ldv, double* __restrict__ vnext, int64_t n)
+{
+    __shared__ double s_inv;
+    const int r = blockIdx.y, nblk = gridDim.x;
+    if (threadIdx.x < 32) {
+        double s = 0.0;                              // one warp: fixed-order strided sums, then shuffles
+        for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
+        s = warp_sum(s);
+        if (threadIdx.x == 0) {
+            const double hn = sqrt(s);
+            s_inv = hn > 0.0 ? 1.0 / hn : 0.0;
+            if (blockIdx.x == 0) hessenberg_update(st, r, j, hn);
+        }
+    }
+    __syncthreads();
+    const double inv = s_inv;
+    int64_t lo, hi; chunk_of(n, lo, hi);
+    const double* wr = w + (int64_t)r * ldv; double* o = vnext + (int64_t)r * ldv;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) o[i] = inv * wr[i];
 }
 
 // beta = sqrt(sum partial) at the start of a cycle: g = (beta, 0, ...), scal[0..1] = beta, 1/beta;
@@ -651,11 +713,6 @@ __global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride
     const double* a = in + (int64_t)blockIdx.y * in_stride; float* o = out + (int64_t)blockIdx.y * out_stride;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (float)a[i];
 }
-__global__ void to_double_kernel(const float* __restrict__ in, int64_t in_stride, double* __restrict__ out, int64_t out_stride, int64_t n)
-{
-    const float* a = in + (int64_t)blockIdx.y * in_stride; double* o = out + (int64_t)blockIdx.y * out_stride;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (double)a[i];
-}
 
 }  // namespace
 
@@ -744,11 +801,9 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
         to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N);
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st);
         if (s != RPY_OK) return s;
-        to_double_kernel<<<vgrid(nrhs), 256, 0, st>>>(W.vel32, 3 * N, out, stride, 3 * N);
     }
     const dim3 bg(warp_grid(nb, 128), (unsigned)nrhs);
-    k_apply_kernel<<<bg, 128, 0, st>>>(pos, q, off, in + 3 * N, -1.0, 1.0, out, nb, stride, stride);
-    kt_apply_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, -1.0, 0.0, out + 3 * N, nb, stride, stride);
+    saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, prec == RPY_PREC_F64 ? nullptr : W.vel32, out, N, nb, stride);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -1067,8 +1122,7 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
             update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 0, W.norm_partial);
             dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
             update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 1, W.norm_partial);
-            hessenberg_kernel<<<nrhs, 32, 0, st>>>(W.st, j, W.norm_partial, kVecBlocks);
-            scale_kernel<<<vg, 256, 0, st>>>(W.w, ldv, W.st.scal, 1, W.V + (int64_t)(j + 1) * nrhs * ldv, ldv, n);
+            normalise_kernel<<<vg, kVecThreads, 0, st>>>(W.st, j, W.norm_partial, W.w, ldv, W.V + (int64_t)(j + 1) * nrhs * ldv, n);
             RPY_CUDA_TRY(mark());
             if (j + 1 < restart && n_iter < max_iter) {          // speculative: P^-1 v_{j+1} for the next iteration
                 if ((s = precond_apply(N, nb, d_precond, W.V + (int64_t)(j + 1) * nrhs * ldv, W.z, ldv, nrhs, st)) != RPY_OK) return s;
