@@ -409,11 +409,13 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
 // kernel streams the inverses at memory speed instead of waiting on 2m dependent substitution steps.
 __global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
                                      double* __restrict__ out, int64_t n_blobs, int64_t n_bodies,
-                                     int64_t vec_stride /* between right-hand sides (blockIdx.y) */)
+                                     int64_t vec_stride /* between right-hand sides (blockIdx.y) */,
+                                     float* __restrict__ lam32 /* optional float copy of lambda, [rhs][3 n_blobs] */)
 {
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     in += (int64_t)blockIdx.y * vec_stride; out += (int64_t)blockIdx.y * vec_stride;
+    if (lam32) lam32 += (int64_t)blockIdx.y * 3 * n_blobs;
     const int64_t* hdr = static_cast<const int64_t*>(precond);
     if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
     const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
@@ -471,6 +473,7 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
 #pragma unroll
                 for (int c = 0; c < 6; ++c) s += Y[(size_t)idx[k] * 6 + c] * U[c];
                 t[idx[k]] = s;
+                if (lam32) lam32[3 * b0 + idx[k]] = (float)s;
             }
         }
     }
@@ -791,14 +794,14 @@ inline dim3 vgrid(int nrhs) { return dim3(kVecBlocks, (unsigned)nrhs); }
 // Eq. (11)'s operator; ONE product call with n_rhs = nrhs.  pos32 must hold float(pos) for the fp32 product.
 rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* pos, const double* q,
                   const int64_t* off, double a, double eta, const double* in, double* out, int64_t stride,
-                  int nrhs, const SolveWs& W, cudaStream_t st)
+                  int nrhs, const SolveWs& W, cudaStream_t st, bool lam32_ready = false)
 {
     rpy_status s;
     if (prec == RPY_PREC_F64) {
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, pos, in, stride, out, stride, a, eta, W.mv, W.mv_bytes, st);
         if (s != RPY_OK) return s;
     } else {
-        to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N);
+        if (!lam32_ready) to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N);
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st);
         if (s != RPY_OK) return s;
     }
@@ -809,9 +812,9 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
 }
 
 rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, int64_t stride,
-                         int nrhs, cudaStream_t st)
+                         int nrhs, cudaStream_t st, float* lam32 = nullptr)
 {
-    precond_apply_kernel<<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride);
+    precond_apply_kernel<<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -1064,6 +1067,7 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
     const int64_t n = W.n, ldv = vec_stride(W);
     const int pvec = restart + 1;
     const dim3 vg = vgrid(nrhs);
+    float* const lam32_in_cycle = inner_prec == RPY_PREC_F64 ? nullptr : W.lam32;   // P^-1 also writes float(lambda)
 
     int64_t bad = -1;
     rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
@@ -1113,9 +1117,9 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
         bool z_ready = false;                    // W.z already holds P^-1 v_j (applied speculatively)
         for (int j = 0; j < restart; ++j) {
             const double* vj = W.V + (int64_t)j * nrhs * ldv;
-            if (!z_ready && (s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+            if (!z_ready && (s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st, lam32_in_cycle)) != RPY_OK) return s;
             z_ready = false;
-            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st)) != RPY_OK) return s;
+            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st, lam32_in_cycle != nullptr)) != RPY_OK) return s;
             ++n_iter;
             // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
             dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
@@ -1125,7 +1129,7 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
             normalise_kernel<<<vg, kVecThreads, 0, st>>>(W.st, j, W.norm_partial, W.w, ldv, W.V + (int64_t)(j + 1) * nrhs * ldv, n);
             RPY_CUDA_TRY(mark());
             if (j + 1 < restart && n_iter < max_iter) {          // speculative: P^-1 v_{j+1} for the next iteration
-                if ((s = precond_apply(N, nb, d_precond, W.V + (int64_t)(j + 1) * nrhs * ldv, W.z, ldv, nrhs, st)) != RPY_OK) return s;
+                if ((s = precond_apply(N, nb, d_precond, W.V + (int64_t)(j + 1) * nrhs * ldv, W.z, ldv, nrhs, st, lam32_in_cycle)) != RPY_OK) return s;
                 z_ready = true;
             }
             RPY_CUDA_TRY(read_marked());
