@@ -370,6 +370,31 @@ def time_solve_batch(torch, cfg: int, matvec_prec: str, tol: float, k: int = 8, 
             "solve_ms": ms, "ms_per_iter": ms / max(1, r["n_iter"]), "ms_per_rhs": ms / k}
 
 
+def size_sweep(torch):
+    """Kernel time, product time and FP-pipe fraction of the wall product against N (config-1 recipe at
+    growing N, k = 1): the evidence behind the kernel / tile-size selection."""
+    from paper_1602_02170_b200 import binding, workloads
+    lane = {"f32": SM_COUNT * LANES["f32"] * SM_MAX_GHZ * 1e9, "f64": SM_COUNT * LANES["f64"] * SM_MAX_GHZ * 1e9}
+    rows = []
+    for n in (1000, 2000, 3000, 3584, 4000, 6144, 8000, 10000, 15000, 20000, 30000, 50000, 100000, 172032):
+        w = workloads.config1(seed=0, n=n)
+        for prec, dt in (("f32", torch.float32), ("f64", torch.float64)):
+            pos = torch.from_numpy(w.pos).to(dt).cuda(); lam = torch.from_numpy(w.force).to(dt).cuda()
+            plan = binding.rpy_matvec_launch_plan(prec, n, 1, n)
+            ts = []
+            for _ in range(8):
+                _, ev = binding.rpy_matvec_phases("wall", pos, lam)
+                torch.cuda.synchronize()
+                ts.append((ev[1].elapsed_time(ev[2]), ev[0].elapsed_time(ev[3])))
+            k_ms = min(t[0] for t in ts[2:]); tot = min(t[1] for t in ts[2:])
+            ops, _ = work_per_pair(prec, "wall", 1, plan["symmetric"])
+            rows.append({"n": n, "prec": prec, "symmetric": plan["symmetric"], "tile": plan["tile_sources"],
+                         "n_ctas": plan["n_ctas"], "kernel_us": k_ms * 1e3, "product_us": tot * 1e3,
+                         "gps_kernel": n * n / k_ms / 1e6, "pipe_frac": n * n * ops / (k_ms * 1e-3) / lane[prec]})
+            log(f"[sweep] {rows[-1]}")
+    return rows
+
+
 def run_ours(args):
     import torch
     from paper_1602_02170_b200 import binding, workloads
@@ -519,11 +544,18 @@ def main():
                     help="only time the preconditioned GMRES mobility solve on this rigid-body config "
                          "(--prec f64|f32, or --solve-prec mixed) and print its JSON (profiling aid)")
     ap.add_argument("--solve-prec", choices=["f64", "f32", "mixed"], default="f64")
+    ap.add_argument("--size-sweep", action="store_true",
+                    help="only print kernel/product time and pipe fraction of the wall product against N (profiling aid)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         log("[bench] note: fewer than 3 warm-up steps requested")
     if args.impl == "reference":
         return run_reference(args)
+    if args.size_sweep:
+        import torch
+        torch.cuda.set_device(0)
+        print(json.dumps(size_sweep(torch)), flush=True)
+        return 0
     if args.rigid_solve:
         import torch
         torch.cuda.set_device(0)
