@@ -722,8 +722,38 @@ __global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride
 // =================================================================== host side
 namespace {
 
-thread_local int64_t* t_tables = nullptr;      // host staging of the offset tables (grown on demand)
-thread_local size_t t_tables_cap = 0;
+// mat_off[p] = sum_{p' < p} (3 blobs_{p'})^2 (exclusive scan, one CTA of 1024 threads), mat_off[nb] = total.
+__global__ void matoff_kernel(const int64_t* __restrict__ off, int64_t* __restrict__ mo, int64_t nb)
+{
+    __shared__ long long wsum[32];
+    __shared__ long long carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < nb; base += 1024) {
+        const int64_t i = base + tid;
+        long long v = 0;
+        if (i < nb) { const long long m = 3 * (off[i + 1] - off[i]); v = m * m; }
+        long long incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const long long t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            long long w = wsum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const long long t = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += t; }
+            wsum[lane] = w;                          // inclusive sums of the warps' totals
+        }
+        __syncthreads();
+        const long long before = carry + (warp > 0 ? wsum[warp - 1] : 0);
+        if (i < nb) mo[i] = before + incl - v;
+        __syncthreads();
+        if (tid == 0) carry += wsum[31];
+        __syncthreads();
+    }
+    if (tid == 0) mo[nb] = carry;
+}
 
 inline bool finite_pos(double v) { return v > 0.0 && isfinite(v); }
 inline unsigned warp_grid(int64_t n_bodies, int threads) { return (unsigned)((n_bodies * 32 + threads - 1) / threads); }
@@ -893,29 +923,19 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
     if (!layout_of(n_bodies, h_offsets, L) || L.n_blobs != n_blobs) return RPY_ERR_ARG;
     if (precond_bytes < L.total || ((uintptr_t)d_precond % kAlign) != 0) return RPY_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    // host tables: header, offsets, matrix offsets -> one staging array, copied before returning
-    const size_t words = 4 + 2 * (size_t)(n_bodies + 1);
-    if (t_tables_cap < words) {
-        int64_t* nt = static_cast<int64_t*>(realloc(t_tables, words * sizeof(int64_t)));
-        if (!nt) return RPY_ERR_ARG;
-        t_tables = nt; t_tables_cap = words;
-    }
-    int64_t* hdr = t_tables; int64_t* off = hdr + 4; int64_t* mo = off + (n_bodies + 1);
-    hdr[0] = kMagic; hdr[1] = n_bodies; hdr[2] = n_blobs; hdr[3] = L.total_mat;
-    int64_t acc = 0; size_t smem = 0;
-    for (int64_t p = 0; p <= n_bodies; ++p) {
-        off[p] = h_offsets[p]; mo[p] = acc;
-        if (p < n_bodies) {
-            const int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]);
-            acc += m * m;
-            if (m <= kSmemBodyM) { size_t need = ((size_t)(m | 1) * m + 6 * m) * 8; if (need > smem) smem = need; }
-        }
+    // tables: header (4 words), the caller's offsets copied up as they are, matrix offsets scanned on the device
+    const int64_t hdr[4] = {kMagic, n_bodies, n_blobs, L.total_mat};
+    size_t smem = 0;
+    for (int64_t p = 0; p < n_bodies; ++p) {
+        const int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]);
+        if (m <= kSmemBodyM) { size_t need = ((size_t)(m | 1) * m + 6 * m) * 8; if (need > smem) smem = need; }
     }
     unsigned char* base = static_cast<unsigned char*>(d_precond);
-    RPY_CUDA_TRY(cudaMemcpyAsync(base, hdr, 4 * 8, cudaMemcpyHostToDevice, st));
-    RPY_CUDA_TRY(cudaMemcpyAsync(base + L.offsets_at, off, (size_t)(n_bodies + 1) * 8, cudaMemcpyHostToDevice, st));
-    RPY_CUDA_TRY(cudaMemcpyAsync(base + L.matoff_at, mo, (size_t)(n_bodies + 1) * 8, cudaMemcpyHostToDevice, st));
-    RPY_CUDA_TRY(cudaStreamSynchronize(st));      // the staging array may be reused by the next call
+    RPY_CUDA_TRY(cudaMemcpyAsync(base, hdr, sizeof hdr, cudaMemcpyHostToDevice, st));
+    RPY_CUDA_TRY(cudaMemcpyAsync(base + L.offsets_at, h_offsets, (size_t)(n_bodies + 1) * 8, cudaMemcpyHostToDevice, st));
+    RPY_CUDA_TRY(cudaStreamSynchronize(st));      // hdr and h_offsets have been read: both may go away now
+    matoff_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const int64_t*>(base + L.offsets_at),
+                                     reinterpret_cast<int64_t*>(base + L.matoff_at), n_bodies);
     PrecondView v = view_of(d_precond, n_bodies, n_blobs, L.total_mat);
     const double PI = 3.14159265358979323846;
     const double scale = 1.0 / (6.0 * PI * eta * a);
