@@ -389,3 +389,23 @@ def test_iteration_count_saturates_with_the_number_of_bodies():
     print("iterations, wall-corrected preconditioner:", its, " unbounded:", its_free)
     assert max(its) <= 26 and its[3] - its[2] <= 1 and its[2] - its[1] <= 2
     assert all(f <= 1.5 * w_ + 1 for f, w_ in zip(its_free, its))
+
+
+def test_large_body_takes_the_global_memory_path_with_chunked_columns():
+    """One 300-blob cylinder (m = 900 > 256 threads: the in-place L^-T L^-1 walks its columns in chunks)
+    next to a 15-blob boomerang: inverse, N~ and the preconditioner solve against numpy."""
+    rng = np.random.default_rng(3)
+    cyl = workloads.cylinder_template(n_rings=50, per_ring=6, radius=1.2, spacing=2.0) + np.array([0.0, 0.0, 4.0])
+    boom = workloads.boomerang_template() + np.array([0.0, 30.0, 3.0])
+    pos = np.concatenate([cyl, boom]); off = np.array([0, 300, 315])
+    q = np.array([cyl.mean(axis=0), boom[0]])
+    db = rigid.bodies(dev(pos), dev(q), off)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    inv, nt = rigid.rpy_rigid_precond_get(pc, 0)
+    M = oracle.dense(oracle.WALL, cyl)
+    assert rel(inv.cpu().numpy(), np.linalg.inv(M)) < 1e-8
+    assert rel(nt.cpu().numpy(), origid.body_mobility(oracle.WALL, cyl, q[:1], np.array([0, 300]))) < 1e-8
+    x = rng.standard_normal(pos.shape); y = rng.standard_normal((2, 6))
+    out = rigid.rpy_rigid_precond_apply(pc, dev(np.concatenate([x.ravel(), y.ravel()]))).cpu().numpy()
+    lam_o, U_o = origid.precond_solve(oracle.WALL, pos, q, off, x, y)
+    assert rel(out[:945], lam_o) < 1e-8 and rel(out[945:], U_o) < 1e-8
