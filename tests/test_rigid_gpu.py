@@ -409,3 +409,21 @@ def test_large_body_takes_the_global_memory_path_with_chunked_columns():
     out = rigid.rpy_rigid_precond_apply(pc, dev(np.concatenate([x.ravel(), y.ravel()]))).cpu().numpy()
     lam_o, U_o = origid.precond_solve(oracle.WALL, pos, q, off, x, y)
     assert rel(out[:945], lam_o) < 1e-8 and rel(out[945:], U_o) < 1e-8
+
+
+def test_bodies_that_cannot_resist_a_torque_are_reported():
+    """Reading A18 (pseudo-inverses): a single blob or a straight line of blobs has a singular
+    K^T M^-1 K (no torque about the axis); the build reports RPY_ERR_NOT_SPD for that body instead of
+    returning a meaningless preconditioner."""
+    line = np.array([[2.0 * i, 0.0, 3.0] for i in range(5)])
+    tri = np.array([[0.0, 10.0, 3.0], [2.0, 10.0, 3.0], [0.0, 12.0, 3.5]])
+    pos = np.concatenate([tri, line, [[20.0, 20.0, 4.0]]])
+    # first partition: body 1 is the straight line, body 2 a single blob; second: body 1 is a single blob
+    for off, bad in ((np.array([0, 3, 8, 9]), 1), (np.array([0, 3, 4, 9]), 1)):
+        q = np.array([pos[off[i]:off[i + 1]].mean(axis=0) for i in range(len(off) - 1)])
+        db = rigid.bodies(dev(pos), dev(q), off)
+        with pytest.raises(RpyError) as ei:
+            rigid.rpy_rigid_precond_build(db, "wall")
+        assert ei.value.status == rigid.RPY_ERR_NOT_SPD and f"body {bad}" in str(ei.value)
+    ok = rigid.bodies(dev(tri), dev(tri.mean(axis=0)[None]), np.array([0, 3]))      # three non-collinear blobs are enough
+    rigid.rpy_rigid_precond_build(ok, "wall")
