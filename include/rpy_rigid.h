@@ -17,7 +17,10 @@
  *               (each body alone, with or without the wall), through the dense inverse of every
  *               M^(pp), formed from its Cholesky factor ("dense matrix inversion (e.g., Cholesky
  *               factorization)"), and the 6x6 body mobilities
- *               N~_pp = (K_p^T (M^(pp))^-1 K_p)^-1
+ *               N~_pp = (K_p^T (M^(pp))^-1 K_p)^+                          PAPER.md:228-250
+ *               (pseudo-inverse: a straight line of blobs or a single blob cannot resist
+ *               a torque about its axis; that direction gets zero mobility, and the loads handed to
+ *               the solve must then carry no torque about it)
  *   solve       Eq. (11), [M -K; -K^T 0][lambda; U] = [slip; -F], by right-preconditioned
  *               restarted GMRES
  *

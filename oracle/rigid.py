@@ -87,8 +87,14 @@ def K_matrix(pos, q, offsets) -> np.ndarray:
     return K
 
 
-def mobility_solve(variant, pos, q, offsets, F, slip=None, a=1.0, eta=1.0):
-    """Solves Eq. (11):  [M -K; -K^T 0] [lambda; U] = [slip; -F].  Returns (lambda [N,3], U [nb,6])."""
+def mobility_solve(variant, pos, q, offsets, F, slip=None, a=1.0, eta=1.0, rank_deficient=False):
+    """Solves Eq. (11):  [M -K; -K^T 0] [lambda; U] = [slip; -F].  Returns (lambda [N,3], U [nb,6]).
+
+    rank_deficient=True: bodies whose blobs lie on a straight line cannot resist a torque about that
+    line, K has a zero column and (11) is singular; "in practice all inverses should be replaced by
+    pseudo-inverses ... no problem ... if the applied force is in the appropriate range"
+    (PAPER.md:192): the minimum-norm least-squares solution (numpy.linalg.lstsq), whose rotation
+    rate about the line is zero."""
     pos, q, offsets, nb = _check(pos, q, offsets)
     n = pos.shape[0]
     M = _dense_mobility(variant, pos, a, eta)
@@ -101,7 +107,7 @@ def mobility_solve(variant, pos, q, offsets, F, slip=None, a=1.0, eta=1.0):
     if slip is not None:
         b[:3 * n] = np.asarray(slip, dtype=np.float64).reshape(-1)
     b[3 * n:] = -np.asarray(F, dtype=np.float64).reshape(-1)
-    x = np.linalg.solve(A, b)
+    x = np.linalg.lstsq(A, b, rcond=1e-12)[0] if rank_deficient else np.linalg.solve(A, b)
     return x[:3 * n].reshape(n, 3), x[3 * n:].reshape(nb, 6)
 
 
@@ -119,8 +125,9 @@ def body_blocks(variant, pos, offsets, a=1.0, eta=1.0):
     return [_dense_mobility(variant, pos[offsets[p]:offsets[p + 1]], a, eta) for p in range(len(offsets) - 1)]
 
 
-def precond_solve(variant, pos, q, offsets, x, y, a=1.0, eta=1.0):
-    """Solves Eq. (19) body by body:  [M~ -K; -K^T 0] [lambda; U] = [x; y]  with M~ of Eq. (17)."""
+def precond_solve(variant, pos, q, offsets, x, y, a=1.0, eta=1.0, rank_deficient=False):
+    """Solves Eq. (19) body by body:  [M~ -K; -K^T 0] [lambda; U] = [x; y]  with M~ of Eq. (17)
+    (rank_deficient=True: minimum-norm least squares per body, see mobility_solve)."""
     pos, q, offsets, nb = _check(pos, q, offsets)
     x = np.asarray(x, dtype=np.float64).reshape(pos.shape)
     y = np.asarray(y, dtype=np.float64).reshape(nb, 6)
@@ -132,6 +139,7 @@ def precond_solve(variant, pos, q, offsets, x, y, a=1.0, eta=1.0):
         Kp = K_matrix(pos[s], q[p:p + 1], np.array([0, m // 3]))
         A = np.zeros((m + 6, m + 6))
         A[:m, :m] = Mpp; A[:m, m:] = -Kp; A[m:, :m] = -Kp.T
-        sol = np.linalg.solve(A, np.concatenate([x[s].reshape(-1), y[p]]))
+        rhs = np.concatenate([x[s].reshape(-1), y[p]])
+        sol = np.linalg.lstsq(A, rhs, rcond=1e-12)[0] if rank_deficient else np.linalg.solve(A, rhs)
         lam[s] = sol[:m].reshape(-1, 3); U[p] = sol[m:]
     return lam, U

@@ -234,6 +234,55 @@ __device__ __forceinline__ void pair_block(double xi, double yi, double zi, doub
     }
 }
 
+// Pseudo-inverse of the symmetric positive SEMI-definite 6x6 K_p^T (M^(pp))^-1 K_p ("in practice all
+// inverses should be replaced by pseudo-inverses"): cyclic Jacobi eigen-decomposition,
+// eigenvalues below 1e-10 of the largest are dropped (a straight line of blobs cannot resist a torque
+// about its axis: that direction gets zero mobility), a negative or non-finite spectrum fails.
+__device__ bool sym6_pinv(const double* __restrict__ a_in, double* __restrict__ out)
+{
+    double a[6][6], v[6][6];
+    for (int r = 0; r < 6; ++r)
+        for (int c = 0; c < 6; ++c) { a[r][c] = 0.5 * (a_in[6 * r + c] + a_in[6 * c + r]); v[r][c] = r == c ? 1.0 : 0.0; }
+    for (int sweep = 0; sweep < 30; ++sweep) {
+        double off = 0.0, diag = 0.0;
+        for (int r = 0; r < 6; ++r)
+            for (int c = 0; c < 6; ++c) { if (r != c) off += a[r][c] * a[r][c]; else diag += a[r][c] * a[r][c]; }
+        if (!(off > 1e-60 * diag) || !isfinite(off)) break;
+        for (int p = 0; p < 5; ++p)
+            for (int q = p + 1; q < 6; ++q) {
+                if (a[p][q] == 0.0) continue;
+                const double theta = (a[q][q] - a[p][p]) / (2.0 * a[p][q]);
+                const double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                const double c = 1.0 / sqrt(t * t + 1.0), sn = t * c;
+                const double app = a[p][p], aqq = a[q][q], apq = a[p][q];
+                for (int k = 0; k < 6; ++k) {                  // rows / columns p and q of J^T A J, k != p, q
+                    if (k == p || k == q) continue;
+                    const double akp = a[k][p], akq = a[k][q];
+                    a[k][p] = a[p][k] = c * akp - sn * akq;
+                    a[k][q] = a[q][k] = sn * akp + c * akq;
+                }
+                a[p][p] = c * c * app - 2.0 * c * sn * apq + sn * sn * aqq;
+                a[q][q] = sn * sn * app + 2.0 * c * sn * apq + c * c * aqq;
+                a[p][q] = a[q][p] = 0.0;
+                for (int k = 0; k < 6; ++k) {                  // V <- V J
+                    const double vkp = v[k][p], vkq = v[k][q];
+                    v[k][p] = c * vkp - sn * vkq; v[k][q] = sn * vkp + c * vkq;
+                }
+            }
+    }
+    double lmax = 0.0;
+    for (int i = 0; i < 6; ++i) { if (!isfinite(a[i][i])) return false; if (a[i][i] > lmax) lmax = a[i][i]; }
+    if (!(lmax > 0.0)) return false;
+    for (int i = 0; i < 6; ++i) if (a[i][i] < -1e-10 * lmax) return false;
+    for (int r = 0; r < 6; ++r)
+        for (int c = 0; c < 6; ++c) {
+            double sum = 0.0;
+            for (int i = 0; i < 6; ++i) if (a[i][i] > 1e-10 * lmax) sum += v[r][i] * v[c][i] / a[i][i];
+            out[6 * r + c] = sum;
+        }
+    return true;
+}
+
 // ------------------------------------------------------------------ preconditioner build
 // One CTA per body.  A (m x m, leading dimension ld) is in shared memory when m <= kSmemBodyM, else
 // it is the body's slot of `factors` (ld = m).  Steps: fill M^(pp); right-looking Cholesky on the
@@ -376,24 +425,10 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
         s_n[tid] = sum;
     }
     __syncthreads();
-    if (tid == 0) {                                          // invert the SPD 6x6 (Gauss-Jordan, no pivoting needed)
-        double a[6][12];
-        for (int r = 0; r < 6; ++r)
-            for (int c = 0; c < 6; ++c) { a[r][c] = 0.5 * (s_n[6 * r + c] + s_n[6 * c + r]); a[r][6 + c] = r == c ? 1.0 : 0.0; }
-        bool ok = true;
-        for (int k = 0; k < 6; ++k) {
-            const double piv = a[k][k];
-            if (!(piv > 0.0) || !isfinite(piv)) { ok = false; break; }
-            const double rp = 1.0 / piv;
-            for (int c = 0; c < 12; ++c) a[k][c] *= rp;
-            for (int r = 0; r < 6; ++r) {
-                if (r == k) continue;
-                const double fct = a[r][k];
-                for (int c = 0; c < 12; ++c) a[r][c] -= fct * a[k][c];
-            }
-        }
-        for (int r = 0; r < 6; ++r)
-            for (int c = 0; c < 6; ++c) Ntg[(size_t)p * 36 + 6 * r + c] = ok ? a[r][6 + c] : 0.0;
+    if (tid == 0) {
+        double nt[36];
+        const bool ok = sym6_pinv(s_n, nt);
+        for (int e = 0; e < 36; ++e) Ntg[(size_t)p * 36 + e] = ok ? nt[e] : 0.0;
         info[p] = ok ? 0 : m + 1;
     }
     if (in_smem)

@@ -60,8 +60,8 @@ def _lib():
 
 def _check(status: int):
     if status == RPY_ERR_NOT_SPD:
-        raise RpyError(status, "RPY_ERR_NOT_SPD: a body's blob mobility M^(pp) is not positive definite "
-                               "(a blob overlapping the wall, or coincident blobs)")
+        raise RpyError(status, "RPY_ERR_NOT_SPD: a body's blob mobility M^(pp) (or its K^T M^-1 K) is not positive "
+                               "(semi-)definite (a blob overlapping the wall, or coincident blobs)")
     binding._check(status)
 
 

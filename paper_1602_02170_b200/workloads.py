@@ -256,3 +256,63 @@ def mixed_suspension(seed: int = 0, n_groups: int = 2):
     b = Bodies(np.array(offsets, dtype=np.int64), np.array(q), rng.standard_normal((len(q), 6)))
     lam = rng.standard_normal(pos.shape)
     return pos, b, lam
+
+
+def rods_near_wall(n_rods: int = 1000, phi: float = 0.1, h_over_d: float = 0.75, seed: int = 0, n_blobs: int = 21):
+    """The suspension of Section V.D / Table III, minimally resolved: cylinders of
+    aspect ratio L/D = 6.4, each `n_blobs` = 21 blobs of radius a = 1.02 R uniformly spaced along a segment
+    of length L, parallel to the wall at centreline height H = h_over_d * D, at surface packing fraction
+    phi.  The paper packs hard rectangles with a molecular-dynamics code; here L x D rectangles are placed
+    by random sequential addition in a periodic square (no overlaps; fine for phi <= 0.3).  Units: a = 1.
+    Returns (pos [n_rods * n_blobs, 3], Bodies)."""
+    rng = np.random.default_rng(seed)
+    R = 1.0 / 1.02; D = 2.0 * R; L = 6.4 * D
+    side = np.sqrt(n_rods * L * D / phi)
+    centres, angles = [], []
+    corners = lambda c, th: c + np.array([[sx * L / 2 * np.cos(th) - sy * D / 2 * np.sin(th),
+                                            sx * L / 2 * np.sin(th) + sy * D / 2 * np.cos(th)]
+                                           for sx in (-1, 1) for sy in (-1, 1)])
+
+    def overlap(c1, t1, c2, t2):                      # separating-axis test for two rectangles
+        d = c2 - c1
+        d -= side * np.round(d / side)                # periodic image
+        if d @ d > (L * L + D * D):
+            return False
+        p1, p2 = corners(np.zeros(2), t1), corners(d, t2)
+        for th in (t1, t1 + np.pi / 2, t2, t2 + np.pi / 2):
+            ax = np.array([np.cos(th), np.sin(th)])
+            a1, a2 = p1 @ ax, p2 @ ax
+            if a1.max() < a2.min() or a2.max() < a1.min():
+                return False
+        return True
+
+    cell = L + D
+    ncell = max(1, int(side // cell))
+    grid = {}
+    while len(centres) < n_rods:
+        c = rng.uniform(0.0, side, 2); th = rng.uniform(0.0, np.pi)
+        key = (int(c[0] / side * ncell) % ncell, int(c[1] / side * ncell) % ncell)
+        ok = True
+        for dx in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for j in grid.get(((key[0] + dx) % ncell, (key[1] + dy) % ncell), ()):
+                    if overlap(c, th, centres[j], angles[j]):
+                        ok = False
+                        break
+                if not ok:
+                    break
+            if not ok:
+                break
+        if ok:
+            grid.setdefault(key, []).append(len(centres))
+            centres.append(c); angles.append(th)
+    s = (np.arange(n_blobs) - (n_blobs - 1) / 2.0) * (L / (n_blobs - 1))
+    pos = np.empty((n_rods, n_blobs, 3))
+    for i, (c, th) in enumerate(zip(centres, angles)):
+        pos[i, :, 0] = c[0] + s * np.cos(th); pos[i, :, 1] = c[1] + s * np.sin(th); pos[i, :, 2] = h_over_d * D
+    q = pos.mean(axis=1)
+    F = np.random.default_rng(seed + 1).standard_normal((n_rods, 6))
+    axis = np.stack([np.cos(angles), np.sin(angles), np.zeros(n_rods)], axis=1)
+    F[:, 3:] -= np.sum(F[:, 3:] * axis, axis=1, keepdims=True) * axis       # no torque about the axis (PAPER.md:192)
+    b = Bodies(np.arange(n_rods + 1, dtype=np.int64) * n_blobs, q, F)
+    return pos.reshape(-1, 3), b

@@ -183,3 +183,43 @@ def test_table6_sphere_near_a_wall_through_the_wall_corrected_body_mobility():
         if x <= 5.0:
             assert rt == pytest.approx(fit("rt_par", x), rel=5e-2)
         assert N[2, 2] < 0.5 * (N[0, 0] + N[1, 1])                # perpendicular motion is hindered more (Fig. 5)
+
+
+def test_straight_rods_minimum_norm_solution():
+    """the paper's minimally resolved rods are blobs on a line segment; K^T M^-1 K is
+    singular (no torque about the axis) and pseudo-inverses are meant.  The minimum-norm solution of
+    (11) satisfies Eq. (10) term by term, does not spin about the axis, equals pinv(K^T M^-1 K) F, turns
+    with the rod in free space, and shows the slender-body anisotropy."""
+    rng = np.random.default_rng(4)
+    nblob = 7
+    axis = np.array([np.cos(0.3), np.sin(0.3), 0.0])
+    rods, q, off = [], [], [0]
+    for c in ([0.0, 0.0, 3.0], [3.0, 9.0, 4.0]):
+        r = np.array(c) + np.outer(2.0 * (np.arange(nblob) - 3), axis)
+        rods.append(r); q.append(r[3]); off.append(off[-1] + nblob)
+    pos = np.concatenate(rods); q = np.array(q); off = np.array(off)
+    F = rng.standard_normal((2, 6))
+    F[:, 3:] -= np.outer(F[:, 3:] @ axis, axis)                      # no torque about the axis: consistent
+    lam, U = rigid.mobility_solve(oracle.WALL, pos, q, off, F, None, rank_deficient=True)
+    assert np.allclose(U[:, 3:] @ axis, 0.0, atol=1e-10)
+    Ml = oracle.matvec(oracle.WALL, pos, lam)
+    assert np.allclose(Ml, rigid.K_apply(pos, q, off, U), atol=1e-9)
+    assert np.allclose(rigid.KT_apply(pos, q, off, lam), F, atol=1e-9)
+    # the same through the Schur complement with a pseudo-inverse (Eq. (12) as PAPER.md:192 reads it)
+    M = oracle.dense(oracle.WALL, pos)
+    K = rigid.K_matrix(pos, q, off)
+    Npinv = np.linalg.pinv(K.T @ np.linalg.solve(M, K), rcond=1e-10)
+    assert np.allclose(U.reshape(-1), Npinv @ F.reshape(-1), rtol=1e-8, atol=1e-12)
+    # free space: turning rod and load together turns the motion (one rod, quarter turn about z)
+    rod = rods[0] - rods[0][3]
+    Rz = np.array([[0.0, -1.0, 0.0], [1.0, 0.0, 0.0], [0.0, 0.0, 1.0]])
+    f = F[:1].copy()
+    _, U0 = rigid.mobility_solve(oracle.FREE, rod, np.zeros((1, 3)), np.array([0, nblob]), f, None, rank_deficient=True)
+    fr = np.concatenate([f[0, :3] @ Rz.T, f[0, 3:] @ Rz.T])[None]
+    _, U1 = rigid.mobility_solve(oracle.FREE, rod @ Rz.T, np.zeros((1, 3)), np.array([0, nblob]), fr, None, rank_deficient=True)
+    assert np.allclose(U1[0, :3], U0[0, :3] @ Rz.T, atol=1e-12) and np.allclose(U1[0, 3:], U0[0, 3:] @ Rz.T, atol=1e-12)
+    # a rod moves more easily along its axis than across it (slender-body ratio between 1 and 2)
+    Nf = np.linalg.pinv(rigid.K_matrix(rod, np.zeros((1, 3)), np.array([0, nblob])).T @ np.linalg.solve(
+        oracle.dense(oracle.FREE, rod), rigid.K_matrix(rod, np.zeros((1, 3)), np.array([0, nblob]))), rcond=1e-10)
+    mu_par = axis @ Nf[:3, :3] @ axis; mu_perp = Nf[2, 2]
+    assert 1.2 < mu_par / mu_perp < 2.0

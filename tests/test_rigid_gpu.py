@@ -411,19 +411,66 @@ def test_large_body_takes_the_global_memory_path_with_chunked_columns():
     assert rel(out[:945], lam_o) < 1e-8 and rel(out[945:], U_o) < 1e-8
 
 
-def test_bodies_that_cannot_resist_a_torque_are_reported():
-    """Reading A18 (pseudo-inverses): a single blob or a straight line of blobs has a singular
-    K^T M^-1 K (no torque about the axis); the build reports RPY_ERR_NOT_SPD for that body instead of
-    returning a meaningless preconditioner."""
-    line = np.array([[2.0 * i, 0.0, 3.0] for i in range(5)])
-    tri = np.array([[0.0, 10.0, 3.0], [2.0, 10.0, 3.0], [0.0, 12.0, 3.5]])
-    pos = np.concatenate([tri, line, [[20.0, 20.0, 4.0]]])
-    # first partition: body 1 is the straight line, body 2 a single blob; second: body 1 is a single blob
-    for off, bad in ((np.array([0, 3, 8, 9]), 1), (np.array([0, 3, 4, 9]), 1)):
-        q = np.array([pos[off[i]:off[i + 1]].mean(axis=0) for i in range(len(off) - 1)])
-        db = rigid.bodies(dev(pos), dev(q), off)
-        with pytest.raises(RpyError) as ei:
-            rigid.rpy_rigid_precond_build(db, "wall")
-        assert ei.value.status == rigid.RPY_ERR_NOT_SPD and f"body {bad}" in str(ei.value)
-    ok = rigid.bodies(dev(tri), dev(tri.mean(axis=0)[None]), np.array([0, 3]))      # three non-collinear blobs are enough
-    rigid.rpy_rigid_precond_build(ok, "wall")
+def test_straight_rods_and_single_blobs_through_the_pseudo_inverse():
+    """Reading A18: the paper's minimally resolved rods are blobs on a line; such a body
+    (and a single blob) cannot resist a torque about its axis, K^T M^-1 K is singular and the 6x6 body
+    mobility is its pseudo-inverse.  With a consistent load (no torque about the axis) the solve returns
+    the minimum-norm solution of (11): the oracle's lstsq solve."""
+    rng = np.random.default_rng(4)
+    nblob = 21
+    rods, q, off, axes = [], [], [0], []
+    for c, ang in (([0.0, 0.0, 3.0], 0.3), ([9.0, 30.0, 4.0], 1.2), ([40.0, 5.0, 2.5], 2.0)):
+        ax = np.array([np.cos(ang), np.sin(ang), 0.0])
+        r = np.array(c) + np.outer(2.0 * (np.arange(nblob) - 10), ax)
+        rods.append(r); q.append(r[10]); off.append(off[-1] + nblob); axes.append(ax)
+    rods.append(np.array([[20.0, 60.0, 3.0]])); q.append(rods[-1][0]); off.append(off[-1] + 1); axes.append(None)   # a single blob
+    pos = np.concatenate(rods); q = np.array(q); off = np.array(off)
+    F = rng.standard_normal((4, 6))
+    for i, ax in enumerate(axes):
+        F[i, 3:] = 0.0 if ax is None else F[i, 3:] - (F[i, 3:] @ ax) * ax
+    db = rigid.bodies(dev(pos), dev(q), off)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    for p in range(3):
+        _, nt = rigid.rpy_rigid_precond_get(pc, p)
+        s = slice(off[p], off[p + 1])
+        Kp = origid.K_matrix(pos[s], q[p:p + 1], np.array([0, nblob]))
+        ref = np.linalg.pinv(Kp.T @ np.linalg.solve(oracle.dense(oracle.WALL, pos[s]), Kp), rcond=1e-10)
+        assert rel(nt.cpu().numpy(), ref) < 1e-8
+    r = rigid.rpy_rigid_mobility_solve(db, pc, dev(F), None, "wall", tol=1e-11)
+    lam_o, U_o = origid.mobility_solve(oracle.WALL, pos, q, off, F, None, rank_deficient=True)
+    assert r["rel_resid"] <= 1e-11
+    assert rel(r["U"].cpu().numpy(), U_o) < 1e-7 and rel(r["lambda"].cpu().numpy(), lam_o) < 1e-6
+    for i, ax in enumerate(axes[:3]):
+        assert abs(r["U"][i, 3:].cpu().numpy() @ ax) < 1e-9 * np.abs(U_o).max()      # no spin about the axis
+    assert not r["U"][3, 3:].any()                                                  # the single blob does not rotate
+
+
+def test_table3_iteration_counts_of_the_rod_suspension():
+    """Table III with the paper's own minimally resolved rods (21 blobs of radius 1.02 R on
+    a segment, aspect ratio 6.4, parallel to the wall), random force/torque and slip on
+    every rod, GMRES to 1e-8.  The packings are ours (random sequential addition instead of the paper's
+    hard-rectangle MD), so the counts are compared within +-3: measured 18 / 23 (paper 19 / 23) at
+    phi = 0.1, 19 / 24 (20 / 25) at phi = 0.2 with the wall-corrected / unbounded preconditioner, 16 (16)
+    at H/D = 2, 15 (14) for 100 rods; phi = 0.4 gives 25 / 29 (25 / 29) but takes 20 s to pack."""
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "table3_iterations.txt"))
+            if l.strip() and l[0] != "#"]
+    want = {}
+    for r in rows:                                            # the left table (both preconditioners) comes first
+        want.setdefault((float(r[1]), int(r[2]), float(r[3])), (int(r[4]), int(r[5])))
+    for phi, nr, hd in ((0.1, 1000, 0.75), (0.2, 1000, 0.75), (0.1, 1000, 2.0), (0.1, 100, 0.75)):
+        pos, hb = workloads.rods_near_wall(nr, phi, hd, seed=0)
+        db = rigid.bodies(dev(pos), dev(hb.q), hb.offsets)
+        slip = dev(0.1 * np.random.default_rng(8).standard_normal(pos.shape))
+        got = []
+        for pv in ("wall", "free"):
+            pc = rigid.rpy_rigid_precond_build(db, pv)
+            r = rigid.rpy_rigid_mobility_solve(db, pc, dev(hb.F), slip, "wall", tol=1e-8)
+            assert r["rel_resid"] <= 1e-8
+            got.append(r["n_iter"])
+        paper = want[(phi, nr, hd)]
+        print(f"phi={phi} rods={nr} H/D={hd}: iterations {got[0]} / {got[1]}, paper {paper[0]} / {paper[1]}")
+        assert abs(got[0] - paper[0]) <= 3
+        if paper[1] > 0:
+            assert abs(got[1] - paper[1]) <= 3
+        assert got[1] <= 1.5 * got[0] + 1                     # "this increase never exceeds 50 %" (PAPER.md:645)
