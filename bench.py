@@ -395,6 +395,30 @@ def size_sweep(torch):
     return rows
 
 
+def time_table3(torch, n_rods: int, matvec_prec: str, paper_iters: int, paper_seconds: float):
+    """Table III (right): the paper's 21-blob rods at phi = 0.1, H/D = 0.75, GMRES to 1e-8
+    with the wall-corrected preconditioner; the paper's iteration count and its Tesla K20 wall-clock time
+    are quoted as context (another machine, another packing)."""
+    from paper_1602_02170_b200 import rigid, workloads
+    pos, hb = workloads.rods_near_wall(n_rods, 0.1, 0.75, seed=0)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=np.float64)).to(dev)
+    b = rigid.bodies(t(pos), t(hb.q), hb.offsets)
+    slip = t(0.1 * np.random.default_rng(8).standard_normal(pos.shape))
+    F = t(hb.F)
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    pc = rigid.rpy_rigid_precond_build(b, "wall")
+    torch.cuda.synchronize(); build_ms = (time.perf_counter() - t0) * 1e3
+    run = lambda: rigid.rpy_rigid_mobility_solve(b, pc, F, slip, "wall", tol=1e-8, matvec_prec=matvec_prec)
+    run(); torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = run()
+    ms = (time.perf_counter() - t0) * 1e3
+    return {"workload": f"table3_rods{n_rods}x21_phi0.1_HD0.75", "n_blobs": b.n_blobs, "n_bodies": n_rods,
+            "matvec_prec": matvec_prec, "n_iter": r["n_iter"], "rel_resid": r["rel_resid"], "solve_ms": ms,
+            "precond_build_ms": build_ms, "paper_iterations": paper_iters, "paper_seconds_tesla_k20": paper_seconds}
+
+
 def run_ours(args):
     import torch
     from paper_1602_02170_b200 import binding, workloads
@@ -521,6 +545,14 @@ def run_ours(args):
                 except Exception as e:  # pragma: no cover
                     batch.append({"config": cfg, "matvec_prec": p, "error": repr(e)})
             line["rigid_solve_batch"] = batch
+            t3 = []
+            for nr, p, it, sec in ((1000, "f64", 19, 32.7), (1000, "mixed", 19, 32.7), (10000, "mixed", 20, 2050.0)):
+                try:
+                    t3.append(time_table3(torch, nr, p, it, sec))
+                    log(f"[bench] table III {t3[-1]}")
+                except Exception as e:  # pragma: no cover
+                    t3.append({"n_rods": nr, "matvec_prec": p, "error": repr(e)})
+            line["table3_rods"] = t3
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
