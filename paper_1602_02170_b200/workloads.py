@@ -316,3 +316,20 @@ def rods_near_wall(n_rods: int = 1000, phi: float = 0.1, h_over_d: float = 0.75,
     F[:, 3:] -= np.sum(F[:, 3:] * axis, axis=1, keepdims=True) * axis       # no torque about the axis
     b = Bodies(np.arange(n_rods + 1, dtype=np.int64) * n_blobs, q, F)
     return pos.reshape(-1, 3), b
+
+
+def sphere_lattice(n_side: int = 8, n_blobs: int = 42, phi: float = 0.09, seed: int = 0):
+    """Section IV.D / Table I (right): n_side^3 spherical shells of `n_blobs` blobs
+    (a/s = 1/2, geometric radius R_g = 1) on a finite simple cubic lattice in an unbounded fluid, at volume
+    fraction phi = (4/3) pi R_h^3 / d^3 (d = lattice spacing; phi = 0.09 is d = 4 R_g = 3.6 R_h).
+    Returns (pos, Bodies, a): random forces and torques on every sphere; the blob radius a."""
+    rh_over_rg = {12: 1.2625, 42: 1.1220}[n_blobs]            # Table I (left), a/s = 1/2
+    t = shell_template(n_blobs)
+    dmat = np.linalg.norm(t[:, None] - t[None], axis=2)
+    a = 0.5 * dmat[dmat > 1e-9].min()
+    d = rh_over_rg * (4.0 * np.pi / (3.0 * phi)) ** (1.0 / 3.0)
+    g = (np.arange(n_side) - (n_side - 1) / 2.0) * d
+    c = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    pos = (c[:, None, :] + t[None, :, :]).reshape(-1, 3)
+    F = np.random.default_rng(seed).standard_normal((c.shape[0], 6))
+    return pos, Bodies(np.arange(c.shape[0] + 1, dtype=np.int64) * n_blobs, c, F), a
