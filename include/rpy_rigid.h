@@ -44,7 +44,7 @@
 extern "C" {
 #endif
 
-#define RPY_RIGID_MAX_BODY_BLOBS 512
+#define RPY_RIGID_MAX_BODY_BLOBS 1024
 #define RPY_RIGID_MAX_RESTART 128
 #define RPY_RIGID_MAX_BATCH 8
 

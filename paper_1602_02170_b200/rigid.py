@@ -18,7 +18,7 @@ from .binding import RPY_PREC_F64, RPY_PREC_F32_ACC64, RpyError, _prec_code  # n
 
 RPY_ERR_NOT_SPD = 6
 RPY_PREC_MIXED = 2       # solve only: fp32 products inside a cycle, fp64 residual per cycle
-RPY_RIGID_MAX_BODY_BLOBS = 512
+RPY_RIGID_MAX_BODY_BLOBS = 1024
 RPY_RIGID_MAX_RESTART = 128
 RPY_RIGID_MAX_BATCH = 8
 

@@ -65,24 +65,24 @@ def icosahedron_vertices() -> np.ndarray:
 
 
 def shell_template(n_blobs: int = 42) -> np.ndarray:
-    """Unit-sphere shell of 12 or 42 blobs: icosahedron vertices, plus (42) the 30 edge
-    midpoints projected back to the sphere (one subdivision)."""
+    """Unit-sphere shell of 12, 42, 162 or 642 blobs: icosahedron vertices, then every subdivision adds the
+    edge midpoints projected back to the sphere.  New points are appended after
+    the old ones, so the 12- and 42-blob shells are prefixes of the finer ones."""
+    levels = {12: 0, 42: 1, 162: 2, 642: 3}
+    if n_blobs not in levels:
+        raise ValueError("shell_template: 12, 42, 162 or 642 blobs")
     v = icosahedron_vertices()
-    if n_blobs == 12:
-        return v
-    if n_blobs != 42:
-        raise ValueError("shell_template: 12 or 42 blobs")
-    d = np.linalg.norm(v[:, None, :] - v[None, :, :], axis=2)
-    edge = d[d > 1e-9].min()
-    mids = []
-    for i in range(12):
-        for j in range(i + 1, 12):
-            if abs(d[i, j] - edge) < 1e-9:
+    for _ in range(levels[n_blobs]):
+        d = np.linalg.norm(v[:, None, :] - v[None, :, :], axis=2)
+        edge = d[d > 1e-9].min()
+        mids = []
+        for i in range(v.shape[0]):
+            for j in np.nonzero((d[i] < 1.2 * edge) & (np.arange(v.shape[0]) > i))[0]:
                 m = 0.5 * (v[i] + v[j])
                 mids.append(m / np.linalg.norm(m))
-    mids = np.array(mids)
-    assert mids.shape == (30, 3)
-    return np.concatenate([v, mids], axis=0)
+        v = np.concatenate([v, np.array(mids)], axis=0)
+    assert v.shape == (n_blobs, 3)
+    return v
 
 
 def boomerang_template() -> np.ndarray:

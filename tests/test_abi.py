@@ -199,7 +199,7 @@ def test_rigid_host_arithmetic_and_argument_checks():
     pb = rigid.rpy_rigid_precond_bytes
     assert pb([0, 15, 30]) > 2 * 45 * 45 * 8 and pb([0, 15, 30]) % 256 == 0
     assert pb([0, 15, 57, 117]) > pb([0, 15, 57])
-    assert pb([1, 15]) == 0 and pb([0, 5, 5]) == 0 and pb([0, 600]) == 0     # bad start, empty body, body too large
+    assert pb([1, 15]) == 0 and pb([0, 5, 5]) == 0 and pb([0, 1200]) == 0     # bad start, empty body, body too large
     w = rigid.rpy_rigid_solve_workspace_bytes
     n, nb = 15000, 1000
     assert w("f64", n, nb, 60) >= 65 * (3 * n + 6 * nb) * 8

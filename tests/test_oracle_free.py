@@ -118,12 +118,12 @@ def _body_mobility(pos, a, eta=1.0):
 
 
 def test_p9_table1_effective_radii():
-    """Table I (left): R_h/R_g and R_tau/R_g of 12- and 42-blob shells.
+    """Table I (left): R_h/R_g and R_tau/R_g of 12-, 42-, 162- and 642-blob shells.
     Pins the far branch, the r = 2a boundary (a/s = 1/2 puts neighbours exactly at 2a),
     the r<2a branch is not reached here; also pins the 1/(6 pi eta a) prefactor."""
     from paper_1602_02170_b200.workloads import shell_template
     rows = [l.split() for l in open(os.path.join(GOLDEN, "table1_radii.txt")) if l.strip() and l[0] != "#"]
-    assert len(rows) == 4
+    assert len(rows) == 8
     for nb, a_over_s, rh_exp, rt_exp in rows:
         pos = shell_template(int(nb))                          # R_g = 1
         d = np.linalg.norm(pos[:, None] - pos[None], axis=2)
