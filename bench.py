@@ -58,14 +58,30 @@ WORK = {
     ("f64", "wall"): (54, 10, 83, 18),
     ("f64", "free"): (17, 10, 24, 18),
 }
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/): (config, prec, variant) -> (bytes, file).  Algorithmic bytes of that
-# launch: 172,032 x 24 B of records read + 16 partial slices x 172,032 x 24 B written/accumulated = 70 MB
-# (mostly L2-resident); the point of the figure is that DRAM traffic is ~1e-3 of what an HBM-bound kernel
-# of this duration would move.
-NCU_TRAFFIC = {
-    (3, "f32", "wall"): (8.368128e6 + 10.961152e6, "profiles/r1b_allpairs_sym_cfg3_wall_f32.md"),
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel come from the committed
+# `ncu --set full` captures: profiles/dram_traffic.csv lists (config, prec, variant, kernel, bytes read,
+# bytes written, the summary file the row was copied from).  Algorithmic bytes of the cfg-3 launch:
+# 172,032 x 24 B of records read + 16 partial slices x 172,032 x 24 B written/accumulated = 70 MB (mostly
+# L2-resident); the point of the figure is that DRAM traffic is ~1e-3 of what an HBM-bound kernel of this
+# duration would move.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+TOL = {"f64": 1e-12, "f32": 1e-5}            # north_star: rel-L2 vs the oracle
+PARITY_ROWS = 2048                           # seeded target rows for configs 3-5 (all rows for 1-2)
+
+
+def ncu_traffic(config: int, prec: str, variant: str):
+    """(bytes per launch, source file) of the latest committed capture for this case, else (None, None)."""
+    try:
+        import csv
+        with open(TRAFFIC_CSV) as f:
+            rows = [r for r in csv.DictReader(f)
+                    if int(r["config"]) == config and r["prec"] == prec and r["variant"] == variant]
+        if not rows:
+            return None, None
+        r = rows[-1]
+        return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), r["source"]
+    except Exception:
+        return None, None
 SM_COUNT = 148
 LANES = {"f32": 128, "f64": 64}
 SM_MAX_GHZ = 1.965
@@ -173,11 +189,38 @@ def oracle_sample(wl, variant: str, prec: str, budget_s: float, max_rows: int = 
     n_rows = int(max(cores, min(max_rows, n, budget_s / max(per_row, 1e-9))))
     rows = workloads.sample_rows(n, n_rows, seed=12345)
     t0 = time.perf_counter()
-    oracle.matvec(ov, pos, force, wl.a, wl.eta, rows=rows)
+    ref = oracle.matvec(ov, pos, force, wl.a, wl.eta, rows=rows)
     t = time.perf_counter() - t0
     gps = len(rows) * n / t / 1e9
     desc = f"{len(rows)} seeded target rows x all {n} sources, k={k}, {variant}, float64"
-    return gps, cores, desc, t, len(rows)
+    return gps, cores, desc, t, len(rows), rows, ref
+
+
+def parity_of(u_gpu, ref, rows, prec: str) -> dict:
+    """rel-L2 over all sampled components and the per-blob maximum max_i |du_i| / |u_i| of the CUDA result
+    `u_gpu` [k, N, 3] against the oracle's `ref` [k, len(rows), 3] (north_star's two figures)."""
+    u = u_gpu.detach().cpu().numpy().astype(np.float64)
+    u = u.reshape(-1, u.shape[-2], 3)[:, rows, :]
+    ref = ref.reshape(u.shape)
+    rel = float(np.linalg.norm((u - ref).ravel()) / np.linalg.norm(ref.ravel()))
+    num = np.linalg.norm(u - ref, axis=-1); den = np.linalg.norm(ref, axis=-1)
+    pb = float((num / np.maximum(den, 1e-300)).max())
+    return {"rel_l2": rel, "per_blob_max": pb, "rows": int(len(rows)), "tol": TOL[prec],
+            "ok": bool(np.isfinite(u).all() and rel <= TOL[prec])}
+
+
+def oracle_parity(wl, variant: str, prec: str, u_gpu, n_rows: int = PARITY_ROWS) -> dict:
+    """The oracle on a seeded row sample (all rows when N <= 20,000) against the CUDA result of the timed step."""
+    import oracle
+    from paper_1602_02170_b200 import workloads
+    ov = oracle.WALL if variant == "wall" else oracle.FREE
+    npdt = np.float32 if prec == "f32" else np.float64
+    pos = wl.pos.astype(npdt).astype(np.float64)          # the values that cross the boundary (reading A8)
+    force = wl.force.astype(npdt).astype(np.float64)
+    n = wl.n_blobs
+    rows = np.arange(n, dtype=np.int64) if n <= 20000 else workloads.sample_rows(n, n_rows, seed=2024)
+    ref = oracle.matvec(ov, pos, force, wl.a, wl.eta, rows=rows)
+    return parity_of(u_gpu, ref, rows, prec)
 
 
 def run_reference(args):
@@ -191,7 +234,7 @@ def run_reference(args):
     budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     times, rows_used, cores, desc = [], 0, 1, ""
     for it in range(args.warmup + args.steps):
-        gps, cores, desc, t, nr = oracle_sample(wl, args.variant, args.prec, budget)
+        gps, cores, desc, t, nr, _, _ = oracle_sample(wl, args.variant, args.prec, budget)
         log(f"[reference] step {it}: {gps:.4f} {UNIT} ({t:.2f} s)")
         if it >= args.warmup:
             times.append(t); rows_used = nr
@@ -228,7 +271,8 @@ def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, ran
     work_shards = world > 1 and k == 1
     rows = None if (world == 1 or work_shards) else sharding.shard_rows(n, rank, world)
     ws = torch.empty(binding.rpy_matvec_workspace_bytes(prec, n, k), dtype=torch.uint8, device=dev)
-    out = torch.empty((k, n if rows is None else rows[1], 3), dtype=dt, device=dev)
+    # the partial products of a work shard are float64 on both paths (fp64 accumulation across ranks)
+    out = torch.empty((k, n if rows is None else rows[1], 3), dtype=torch.float64 if work_shards else dt, device=dev)
     gathered = sharding.gather_buffers(n, k, world, dt, dev) if (world > 1 and not work_shards) else None
 
     def step():
@@ -268,12 +312,13 @@ def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, ran
 
 def time_allpairs_kernel(torch, binding, res, wl, variant, steps, flush_buf):
     """CUDA events recorded by the library on its launch stream around the all-pairs kernel."""
+    import bench_aids
     times, pre, fin = [], [], []
     for _ in range(steps):
         if flush_buf is not None:
             flush_buf.zero_()
-        _, ev = binding.rpy_matvec_phases(variant, res["pos"], res["force"], wl.a, wl.eta, out=res["out"],
-                                          workspace=res["ws"])
+        _, ev = bench_aids.matvec_phases(variant, res["pos"], res["force"], wl.a, wl.eta, out=res["out"],
+                                         workspace=res["ws"])
         torch.cuda.synchronize()
         pre.append(ev[0].elapsed_time(ev[1])); times.append(ev[1].elapsed_time(ev[2])); fin.append(ev[2].elapsed_time(ev[3]))
     return float(np.mean(times)), float(np.mean(pre)), float(np.mean(fin))
@@ -373,6 +418,7 @@ def time_solve_batch(torch, cfg: int, matvec_prec: str, tol: float, k: int = 8, 
 def size_sweep(torch):
     """Kernel time, product time and FP-pipe fraction of the wall product against N (config-1 recipe at
     growing N, k = 1): the evidence behind the kernel / tile-size selection."""
+    import bench_aids
     from paper_1602_02170_b200 import binding, workloads
     lane = {"f32": SM_COUNT * LANES["f32"] * SM_MAX_GHZ * 1e9, "f64": SM_COUNT * LANES["f64"] * SM_MAX_GHZ * 1e9}
     rows = []
@@ -383,7 +429,7 @@ def size_sweep(torch):
             plan = binding.rpy_matvec_launch_plan(prec, n, 1, n)
             ts = []
             for _ in range(8):
-                _, ev = binding.rpy_matvec_phases("wall", pos, lam)
+                _, ev = bench_aids.matvec_phases("wall", pos, lam)
                 torch.cuda.synchronize()
                 ts.append((ev[1].elapsed_time(ev[2]), ev[0].elapsed_time(ev[3])))
             k_ms = min(t[0] for t in ts[2:]); tot = min(t[1] for t in ts[2:])
@@ -451,44 +497,55 @@ def run_ours(args):
     instr, flops = work_per_pair(prec, variant, k, plan["symmetric"])
 
     line = None
+    parity_failed = False
     if rank == 0:
-        # --- roofline of the dominant kernel (single-GPU geometry), timed on its own stream
-        if world == 1:
-            k_ms, pre_ms, fin_ms = time_allpairs_kernel(torch, binding, res, wl, variant, max(3, min(args.steps, 10)), flush)
-        else:
-            k_ms, pre_ms, fin_ms = ms, 0.0, 0.0
-        pairs_launch = n * n // world
-        achieved = pairs_launch * flops / (k_ms * 1e-3) / 1e12
-        peak = peak_tflops(prec)
-        # measured FMA-chain rate on this GPU, same run (context for the derived peak)
+        import bench_aids
+        # measured FMA-chain rates on this GPU, same run (context for the derived peak)
         probe = {}
         try:
-            for kind, name in ((0, "ffma"), (1, "ffma2"), (2, "dfma"), (3, "mufu_rsq")):
-                probe[name + "_g_per_s"] = round(binding.rpy_pipe_peak_probe(kind, 8192)["gfma_per_s"], 1)
+            for kind, name in ((0, "ffma"), (1, "ffma2"), (2, "dfma"), (3, "mufu_rsq"), (4, "ffma2_three_reg"), (5, "ffma_three_reg")):
+                probe[name + "_g_per_s"] = round(bench_aids.pipe_probe(kind, 8192)["gfma_per_s"], 1)
         except Exception as e:  # pragma: no cover
             probe = {"error": str(e)}
-        lane_peak = SM_COUNT * LANES[prec] * SM_MAX_GHZ * 1e9
-        roofline = {
-            "bound": "alu", "kernel": "allpairs_sym_kernel" if plan["symmetric"] else "allpairs_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-            "frac": achieved / peak,
-            "traffic": NCU_TRAFFIC.get((args.config, prec, variant), (None, None))[0] if k == 1 else None,
-            "traffic_source": NCU_TRAFFIC.get((args.config, prec, variant), (None, None))[1] if k == 1 else None,
-            "peak_source": f"derived: {SM_COUNT} SM x {LANES[prec]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
-            "flop_per_pair": flops, "lane_ops_per_pair": instr,
-            "pipe_frac": pairs_launch * instr / (k_ms * 1e-3) / lane_peak,
-            "kernel_ms": k_ms, "prepack_ms": pre_ms, "finalise_ms": fin_ms,
-            "kernel_share_of_step": k_ms / (k_ms + pre_ms + fin_ms) if world == 1 else None,
-            "measured_chain_rates": probe,
-        }
+
+        def roofline_of(cfg, p, v, w, r, plan_, kernel_steps):
+            """Roofline object of the dominant kernel of one configuration (single-GPU geometry): the kernel is
+            timed on its own launch stream by CUDA events recorded inside the library call."""
+            ops, fl = work_per_pair(p, v, w.n_rhs, plan_["symmetric"])
+            if world == 1:
+                k_ms, pre_ms, fin_ms = time_allpairs_kernel(torch, binding, r, w, v, kernel_steps, flush)
+            else:
+                k_ms, pre_ms, fin_ms = r["ms_per_step"], 0.0, 0.0
+            pairs_launch = w.n_blobs * w.n_blobs // world
+            achieved = pairs_launch * fl / (k_ms * 1e-3) / 1e12
+            peak = peak_tflops(p)
+            lane_peak = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
+            traffic, src = ncu_traffic(cfg, p, v) if w.n_rhs == 1 else (None, None)
+            return {
+                "bound": "alu", "kernel": "allpairs_sym_kernel" if plan_["symmetric"] else "allpairs_kernel",
+                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": traffic, "traffic_source": src,
+                "peak_source": f"derived: {SM_COUNT} SM x {LANES[p]} lanes x 2 flop x {SM_MAX_GHZ} GHz (DESIGN.md)",
+                "flop_per_pair": fl, "lane_ops_per_pair": ops,
+                "pipe_frac": pairs_launch * ops / (k_ms * 1e-3) / lane_peak,
+                "kernel_ms": k_ms, "prepack_ms": pre_ms, "finalise_ms": fin_ms,
+                "kernel_share_of_step": k_ms / (k_ms + pre_ms + fin_ms) if world == 1 else None,
+            }
+
+        roofline = roofline_of(args.config, prec, variant, wl, res, plan, max(3, min(args.steps, 10)))
+        roofline["measured_chain_rates"] = probe
         # --- end to end through the host-buffer C-ABI call
         e2e = time_e2e(torch, binding, wl, prec, variant, max(2, min(args.steps, 5)), 1) if world == 1 else \
             {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
              "note": "host-buffer call is single-GPU; run with --gpus 1"}
-        # --- the oracle on the host cores, bounded sample
-        cpu = None
+        # --- the oracle on the host cores, bounded sample; its velocities give the parity of the timed step
+        cpu, parity = None, None
         if world == 1 and not args.no_cpu:
-            gps, cores, desc, t, _ = oracle_sample(wl, variant, prec, 15.0)
+            gps, cores, desc, t, _, orows, oref = oracle_sample(wl, variant, prec, 15.0)
             cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
+            parity = parity_of(res["out"], oref, orows, prec)
+            parity_failed = parity_failed or not parity["ok"]
+            log(f"[bench] parity vs oracle: {parity}")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
@@ -504,15 +561,29 @@ def run_ours(args):
                        "launch_plan": plan},
             "pair_rhs_gps": value * k,
             "clocks": clocks, "e2e": e2e, "gpu_launches": 3 * args.steps * (1 if k <= 8 else -(-k // 8)),
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "parity": parity,
         }
+        # --- the paper's own precision ("in double precision"): the fp64 path on the same workload,
+        # in fields of its own so that it is not only a context line
+        if world == 1 and prec == "f32" and not args.no_f64:
+            st64 = max(3, min(args.steps, 5))
+            r64 = time_config(torch, binding, wl, "f64", variant, st64, 3, flush)
+            pl64 = binding.rpy_matvec_launch_plan("f64", n, k, n)
+            line["value_f64"] = r64["gps"]
+            line["ms_per_step_f64"] = r64["ms_per_step"]
+            line["roofline_f64"] = roofline_of(args.config, "f64", variant, wl, r64, pl64, 3)
+            if not args.no_cpu:
+                line["parity_f64"] = oracle_parity(wl, variant, "f64", r64["out"])
+                parity_failed = parity_failed or not line["parity_f64"]["ok"]
+                log(f"[bench] f64: {r64['gps']:.1f} {UNIT}, parity {line['parity_f64']}")
+            del r64
         # --- the other BASELINE.json configurations, fewer steps (context; not the headline)
         if world == 1 and not args.no_extra:
             extra = []
-            for cfg, p, v, st in ((3, "f64", "wall", 3), (5, "f32", "wall", 3), (5, "f32", "free", 3),
+            for cfg, p, v, st in ((5, "f32", "wall", 3), (5, "f32", "free", 3),
                                   (2, "f64", "wall", 10), (2, "f32", "wall", 10), (1, "f64", "wall", 10),
-                                  (4, "f32", "wall", 1)):
-                if (cfg, p, v) == (args.config, prec, variant):
+                                  (4, "f32", "wall", 1), (3, "f64", "wall", 3)):
+                if (cfg, p, v) == (args.config, prec, variant) or ((cfg, v) == (args.config, variant) and "value_f64" in line and p == "f64"):
                     continue
                 w2 = workloads.make(cfg)
                 r2 = time_config(torch, binding, w2, p, v, st, 3 if cfg != 4 else 1, flush)
@@ -520,11 +591,16 @@ def run_ours(args):
                 pl2 = binding.rpy_matvec_launch_plan(p, w2.n_blobs, w2.n_rhs, w2.n_blobs)
                 i2, f2 = work_per_pair(p, v, w2.n_rhs, pl2["symmetric"])
                 lane2 = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
+                par2 = None
+                if not args.no_cpu:
+                    par2 = oracle_parity(w2, v, p, r2["out"])
+                    parity_failed = parity_failed or not par2["ok"]
                 extra.append({"workload": w2.name, "prec": p, "variant": v, "n_blobs": w2.n_blobs, "n_rhs": w2.n_rhs,
                               "ms_per_step": r2["ms_per_step"], "gps": r2["gps"], "pair_rhs_gps": r2["gps"] * w2.n_rhs,
                               "kernel_ms": km, "symmetric": pl2["symmetric"],
                               "pipe_frac": w2.n_blobs ** 2 * i2 / (km * 1e-3) / lane2,
-                              "flop_frac": w2.n_blobs ** 2 * f2 / (km * 1e-3) / 1e12 / peak_tflops(p)})
+                              "flop_frac": w2.n_blobs ** 2 * f2 / (km * 1e-3) / 1e12 / peak_tflops(p),
+                              "parity": par2})
                 log(f"[bench] extra {extra[-1]}")
                 del r2
             line["other_configs"] = extra
@@ -558,6 +634,9 @@ def run_ours(args):
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+        if parity_failed:
+            log("[bench] PARITY FAILURE: a CUDA result is outside north_star's tolerance of the oracle (see 'parity' fields)")
+            return 3
     return 0
 
 
@@ -571,7 +650,8 @@ def main():
     ap.add_argument("--prec", choices=["f32", "f64"], default="f32")
     ap.add_argument("--variant", choices=["wall", "free"], default="wall")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configurations")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle timing and the parity figures")
+    ap.add_argument("--no-f64", action="store_true", help="skip the fp64 path of the headline workload (value_f64, roofline_f64)")
     ap.add_argument("--rigid-solve", type=int, default=0, choices=[0, 2, 3],
                     help="only time the preconditioned GMRES mobility solve on this rigid-body config "
                          "(--prec f64|f32, or --solve-prec mixed) and print its JSON (profiling aid)")

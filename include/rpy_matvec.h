@@ -110,8 +110,10 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
 /* Work-sharded forms: one of n_shards PARTIAL products whose sum over shard = 0 .. n_shards-1 is
  * u = M lambda; the unit a multi-GPU caller gives each rank when it wants the symmetric kernel's
  * halved arithmetic on every GPU (it then adds the partial results with one all-reduce of
- * 3 n_rhs n_blobs elements).  d_vel [n_rhs][n_blobs][3] is overwritten with the shard's contribution
- * to EVERY row.  For n_rhs == 1 and n_blobs >= 3,584 a shard is a contiguous range of the tile
+ * 3 n_rhs n_blobs doubles).  d_vel [n_rhs][n_blobs][3] is overwritten with the shard's contribution
+ * to EVERY row and is DOUBLE on both paths: the cross-shard sum is part of the "fp64 accumulation" of
+ * the fp32 path and must not round to float per shard (pos and force keep the path's type).
+ * For n_rhs == 1 and n_blobs >= 3,584 a shard is a contiguous range of the tile
  * distances of the symmetric kernel (all distances cost the same, so shards are balanced); otherwise
  * it is a contiguous range of target rows of the plain kernel and the other rows are zero.
  * 0 <= shard < n_shards <= 4096.  Workspace: rpy_matvec_workspace_bytes().                        */
@@ -175,29 +177,6 @@ rpy_status rpy_free_matvec_host(rpy_prec prec, int64_t n_blobs, int n_rhs,
  * int64 that is overwritten (zeroed, then accumulated) in stream order. */
 rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void *d_pos, double zmin,
                                 int64_t *d_count, void *cuda_stream);
-
-/* Measurement aid for the ALU roofline: runs a register-only chain
- * of independent fused multiply-adds on every SM and writes the elapsed milliseconds
- * (CUDA events on `cuda_stream`, which is synchronised) to *h_elapsed_ms and the number of
- * scalar FMAs executed to *h_fma_count.  kind: 0 = FFMA (scalar float), 1 = packed
- * fma.rn.f32x2 (two float FMAs per instruction), 2 = DFMA (double), 3 = MUFU.RSQ,
- * 4 = packed f32x2 with three distinct register-pair operands, 5 = FFMA with three distinct
- * register operands (kinds 0-2 multiply by loop-invariant registers).
- * d_sink: device buffer of at least 8 bytes (defeats dead-code elimination). */
-rpy_status rpy_pipe_peak_probe(int kind, int iters, void *d_sink, float *h_elapsed_ms,
-                               double *h_fma_count, void *cuda_stream);
-
-/* Measurement aid: the whole-matrix matvec (wall != 0: wall-corrected, else free space) with
- * four caller-owned CUDA events (cudaEvent_t passed as void*) recorded on `cuda_stream`
- *   [0] before prepack, [1] before the all-pairs kernel, [2] after it, [3] after finalise
- * of the first right-hand-side group (n_rhs <= 8: the only one).  Same arguments, checks and
- * result as rpy_wall_matvec / rpy_free_matvec otherwise; n_blobs >= 1.  bench.py uses it to
- * time the dominant kernel on the stream it is launched on. */
-rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs,
-                             const void *d_pos, const void *d_force, void *d_vel,
-                             double a, double eta,
-                             void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                             void *const *cuda_events4);
 
 /* Launch geometry the all-pairs kernel would use for (prec, n_blobs, n_rhs, row_count).
  * Pure host arithmetic (no CUDA call); any output pointer may be NULL.

@@ -15,7 +15,7 @@ from __future__ import annotations
 __all__ = [
     "rpy_wall_matvec", "rpy_free_matvec", "rpy_wall_matvec_host", "rpy_free_matvec_host",
     "rpy_matvec_workspace_bytes", "rpy_matvec_host_scratch_bytes", "rpy_wall_count_below",
-    "rpy_matvec_launch_plan", "rpy_pipe_peak_probe", "rpy_matvec_phases",
+    "rpy_matvec_launch_plan",
     "rpy_wall_matvec_shard", "rpy_free_matvec_shard", "rpy_wall_matvec_rect", "rpy_free_matvec_rect", "rpy_matvec_rect_workspace_bytes", "rpy_flow_subdivide",
     "rpy_status_string", "RpyError", "load_library", "library_path",
 ]

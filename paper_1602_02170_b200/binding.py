@@ -56,12 +56,8 @@ SIGNATURES = {
     "rpy_wall_matvec_host": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_free_matvec_host": (_int, [_int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp]),
     "rpy_wall_count_below": (_int, [_int, _i64, _vp, _dbl, _vp, _vp]),
-    "rpy_pipe_peak_probe": (_int, [_int, _int, _vp, ctypes.POINTER(ctypes.c_float),
-                                   ctypes.POINTER(ctypes.c_double), _vp]),
     "rpy_matvec_launch_plan": (_int, [_int, _i64, _int, _i64, ctypes.POINTER(_int), ctypes.POINTER(_int),
                                       ctypes.POINTER(_int), ctypes.POINTER(_i64), ctypes.POINTER(_int)]),
-    "rpy_matvec_phases": (_int, [_int, _int, _i64, _int, _vp, _vp, _vp, _dbl, _dbl, _vp, _sz, _vp,
-                                 ctypes.POINTER(_vp)]),
     "rpy_status_string": (ctypes.c_char_p, [_int]),
     "rpy_last_cuda_error": (_int, []),
     "rpy_abi_version": (_int, []),
@@ -229,10 +225,11 @@ def _matvec_shard(fn_name: str, pos, force, shard, n_shards, a, eta, out, worksp
     n, k, single = _shape_inputs(pos, force)
     prec = _prec_of(pos.dtype)
     oshape = (n, 3) if single else (k, n, 3)
+    # partial velocities are float64 on both paths (the cross-shard sum keeps the fp64 accumulation)
     if out is None:
-        out = torch.empty(oshape, dtype=pos.dtype, device=pos.device)
-    elif tuple(out.shape) != oshape or out.dtype != pos.dtype or out.device != pos.device or not out.is_contiguous():
-        raise ValueError(f"out must be a contiguous {pos.dtype} tensor of shape {oshape} on {pos.device}")
+        out = torch.empty(oshape, dtype=torch.float64, device=pos.device)
+    elif tuple(out.shape) != oshape or out.dtype != torch.float64 or out.device != pos.device or not out.is_contiguous():
+        raise ValueError(f"out must be a contiguous float64 tensor of shape {oshape} on {pos.device}")
     ws, ws_bytes = _workspace(prec, n, k, pos.device, workspace)
     with torch.cuda.device(pos.device):
         stream = torch.cuda.current_stream(pos.device).cuda_stream
@@ -244,8 +241,8 @@ def _matvec_shard(fn_name: str, pos, force, shard, n_shards, a, eta, out, worksp
 
 def rpy_wall_matvec_shard(pos: torch.Tensor, force: torch.Tensor, shard: int, n_shards: int, a: float = 1.0,
                           eta: float = 1.0, *, out=None, workspace=None) -> torch.Tensor:
-    """Shard `shard` of `n_shards` of u = M lambda (wall tensor): a partial result for ALL rows; the
-    sum over the shards is the product (multi-GPU: one all-reduce).  Uses the symmetric kernel."""
+    """Shard `shard` of `n_shards` of u = M lambda (wall tensor): a partial result for ALL rows, always
+    float64; the sum over the shards is the product (multi-GPU: one all-reduce).  Uses the symmetric kernel."""
     return _matvec_shard("rpy_wall_matvec_shard", pos, force, shard, n_shards, a, eta, out, workspace)
 
 
@@ -315,36 +312,6 @@ def rpy_flow_subdivide(pos: torch.Tensor, force: torch.Tensor, template: torch.T
     return sub_pos, sub_force
 
 
-def rpy_matvec_phases(variant: str, pos: torch.Tensor, force: torch.Tensor, a: float = 1.0, eta: float = 1.0, *,
-                      out: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
-                      events=None):
-    """Whole-matrix matvec with four CUDA events recorded around its phases (measurement aid).
-
-    Returns (u, events); after synchronising, ``events[1].elapsed_time(events[2])`` is the
-    duration of the all-pairs kernel in ms.
-    """
-    lib = load_library()
-    _require_cuda(pos, "pos")
-    _require_cuda(force, "force")
-    n, k, single = _shape_inputs(pos, force)
-    prec = _prec_of(pos.dtype)
-    oshape = (n, 3) if single else (k, n, 3)
-    if out is None:
-        out = torch.empty(oshape, dtype=pos.dtype, device=pos.device)
-    ws, ws_bytes = _workspace(prec, n, k, pos.device, workspace)
-    with torch.cuda.device(pos.device):
-        if events is None:
-            events = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-            stream0 = torch.cuda.current_stream(pos.device)
-            for e in events:
-                e.record(stream0)         # torch creates the cudaEvent_t lazily, on first record
-        handles = (_vp * 4)(*[e.cuda_event for e in events])
-        stream = torch.cuda.current_stream(pos.device).cuda_stream
-        _check(lib.rpy_matvec_phases(1 if variant == "wall" else 0, prec, n, k, pos.data_ptr(), force.data_ptr(),
-                                     out.data_ptr(), float(a), float(eta), ws.data_ptr(), ws_bytes, stream, handles))
-    return out, events
-
-
 def _matvec_host(fn_name: str, pos, force, a, eta, out, scratch, device):
     lib = load_library()
     if not torch.cuda.is_available():
@@ -394,18 +361,3 @@ def rpy_wall_count_below(pos: torch.Tensor, zmin: float) -> int:
         _check(lib.rpy_wall_count_below(prec, pos.shape[0], pos.data_ptr() or None, float(zmin),
                                         cnt.data_ptr(), stream))
     return int(cnt.item())
-
-
-def rpy_pipe_peak_probe(kind: int, iters: int = 4096, device=None) -> dict:
-    """FMA-chain probe: returns {'ms', 'fma', 'gfma_per_s'} for kind 0 FFMA, 1 FFMA2, 2 DFMA, 3 MUFU.RSQ."""
-    lib = load_library()
-    if not torch.cuda.is_available():
-        raise RuntimeError("rpy_pipe_peak_probe needs a CUDA device")
-    device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-    sink = torch.zeros(8, dtype=torch.float64, device=device)
-    ms, cnt = ctypes.c_float(), ctypes.c_double()
-    with torch.cuda.device(device):
-        stream = torch.cuda.current_stream(device).cuda_stream
-        _check(lib.rpy_pipe_peak_probe(int(kind), int(iters), sink.data_ptr(), ctypes.byref(ms),
-                                       ctypes.byref(cnt), stream))
-    return {"ms": ms.value, "fma": cnt.value, "gfma_per_s": cnt.value / (ms.value * 1e-3) / 1e9}

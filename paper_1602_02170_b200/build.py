@@ -16,7 +16,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "librpy_matvec.so"
-SOURCES = [CSRC / "rpy_matvec.cu", CSRC / "rpy_probe.cu", CSRC / "rpy_rigid.cu"]
+SOURCES = [CSRC / "rpy_matvec.cu", CSRC / "rpy_rigid.cu"]
 DEPS = SOURCES + [CSRC / "rpy_math.cuh", CSRC / "rpy_kernels.cuh", CSRC / "rpy_internal.h",
                INCLUDE / "rpy_matvec.h", INCLUDE / "rpy_rigid.h"]
 

@@ -20,7 +20,7 @@ namespace {
 
 thread_local int g_last_cuda_error = 0;
 
-constexpr int kAbiVersion = 4;
+constexpr int kAbiVersion = 5;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
 constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
 constexpr int kMaxChunks = 64;
@@ -237,11 +237,12 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
 
 template <class L, int K>
 cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
-                      const typename L::S* pos, const typename L::S* force, typename L::S* vel,
+                      const typename L::S* pos, const typename L::S* force, void* vel,
                       double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev,
                       const typename L::S* tpos /* targets of the rectangular product, else nullptr */,
                       Shard sh, int64_t vel_stride3 /* elements between right-hand sides of vel */,
-                      int64_t force_stride3 /* the same for force */)
+                      int64_t force_stride3 /* the same for force */,
+                      bool vel_f64 /* vel is double whatever the path (partial products of a shard) */)
 {
     using S = typename L::S;
     S* rec = reinterpret_cast<S*>(ws);
@@ -293,9 +294,11 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int threads = 256;
         int64_t blocks = (per_chunk + threads - 1) / threads;
         const double PI = 3.14159265358979323846;
-        rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, vel, per_chunk, n_slices,
-                                                                    rows * 3, vel_stride3,
-                                                                    1.0 / (6.0 * PI * eta * a));
+        const double scale = 1.0 / (6.0 * PI * eta * a);
+        if (vel_f64) rpy::finalise_kernel<double><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<double*>(vel), per_chunk, n_slices,
+                                                                                     rows * 3, vel_stride3, scale);
+        else         rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<S*>(vel), per_chunk, n_slices,
+                                                                               rows * 3, vel_stride3, scale);
         e = cudaGetLastError();
     }
     return e;
@@ -306,7 +309,7 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
                            const void* d_pos, const void* d_force, void* d_vel,
                            double a, double eta, void* ws, cudaStream_t st, void* const* ev,
                            const void* d_tpos = nullptr, Shard sh = Shard{0, 1}, int64_t vel_stride3 = -1,
-                           int64_t force_stride3 = -1)
+                           int64_t force_stride3 = -1, bool vel_f64 = false)
 {
     using S = typename L::S;
     cudaError_t ee;
@@ -319,14 +322,14 @@ cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, i
     while (done < n_rhs) {
         int K = group_k(n_rhs - done);
         const S* force = static_cast<const S*>(d_force) + (int64_t)done * force_stride3;
-        S* vel = static_cast<S*>(d_vel) + (int64_t)done * vel_stride3;
+        void* vel = static_cast<unsigned char*>(d_vel) + (size_t)done * vel_stride3 * (vel_f64 ? sizeof(double) : sizeof(S));
         unsigned char* w = static_cast<unsigned char*>(ws);
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
-            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
-            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
-            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
@@ -375,27 +378,28 @@ rpy_status matvec_shard(bool wall, rpy_prec prec, int64_t n, int n_rhs, int shar
     if (!d_pos || !d_force || !d_vel || !ws) return RPY_ERR_NULL;
     size_t es = elem_size(prec);
     size_t pos_b = (size_t)n * 3 * es, force_b = pos_b * (size_t)n_rhs;
+    size_t vel_b = (size_t)n * 3 * sizeof(double) * (size_t)n_rhs;       // partial velocities are double on both paths
     size_t need = workspace_bytes(prec, n, n_rhs);
     if (ws_bytes < need || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
-    if (overlaps(d_vel, force_b, d_pos, pos_b) || overlaps(d_vel, force_b, d_force, force_b) || overlaps(d_vel, force_b, ws, need))
+    if (overlaps(d_vel, vel_b, d_pos, pos_b) || overlaps(d_vel, vel_b, d_force, force_b) || overlaps(d_vel, vel_b, ws, need))
         return RPY_ERR_ALIAS;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
     if (n_rhs == 1 && use_symmetric(n, 1, 0, n)) {
         const Shard sh{shard, n_shards};
         e = prec == RPY_PREC_F64
-            ? run_all_groups<rpy::Lane<double>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh)
-            : run_all_groups<rpy::Lane<float2>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh);
+            ? run_all_groups<rpy::Lane<double>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh, -1, -1, true)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh, -1, -1, true);
     } else {
         const int64_t r0 = n * shard / n_shards, r1 = n * (shard + 1) / n_shards;
-        if ((e = cudaMemsetAsync(d_vel, 0, force_b, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaMemsetAsync(d_vel, 0, vel_b, st)) != cudaSuccess) return cuda_fail(e);
         if (r1 == r0) return RPY_OK;
-        void* out = static_cast<unsigned char*>(d_vel) + (size_t)r0 * 3 * es;
+        void* out = static_cast<unsigned char*>(d_vel) + (size_t)r0 * 3 * sizeof(double);
         // rows r0..r1-1 by the plain kernel (never the symmetric one: row_begin/rows are not the whole range,
         // or n is below the symmetric threshold), written in place of the full-length layout
         e = prec == RPY_PREC_F64
-            ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3)
-            : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3);
+            ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3, -1, true)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3, -1, true);
     }
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
@@ -478,6 +482,14 @@ rpy_status matvec_host(bool wall, rpy_prec prec, int64_t n, int n_rhs, const voi
 
 namespace rpy {
 rpy_status set_cuda_error(cudaError_t e) { return cuda_fail(e); }
+
+rpy_status matvec_phases(bool wall, rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos, const void* d_force,
+                         void* d_vel, double a, double eta, void* ws, size_t ws_bytes, void* stream, void* const* events4)
+{
+    if (!events4 || !events4[0] || !events4[1] || !events4[2] || !events4[3]) return RPY_ERR_NULL;
+    if (n_blobs < 1) return RPY_ERR_ARG;
+    return matvec_rows(wall, prec, n_blobs, n_rhs, 0, n_blobs, d_pos, d_force, d_vel, a, eta, ws, ws_bytes, stream, events4);
+}
 
 rpy_status matvec_strided(bool wall, rpy_prec prec, int64_t n, int n_rhs, const void* d_pos, const void* d_force,
                           int64_t force_stride3, void* d_vel, int64_t vel_stride3, double a, double eta,
@@ -597,17 +609,6 @@ rpy_status rpy_flow_subdivide(rpy_prec prec, int64_t n_blobs, int n_rhs, int n_s
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
-}
-
-rpy_status rpy_matvec_phases(int wall, rpy_prec prec, int64_t n_blobs, int n_rhs, const void* d_pos,
-                             const void* d_force, void* d_vel, double a, double eta, void* d_workspace,
-                             size_t workspace_bytes_, void* cuda_stream, void* const* cuda_events4)
-{
-    if (!cuda_events4 || !cuda_events4[0] || !cuda_events4[1] || !cuda_events4[2] || !cuda_events4[3])
-        return RPY_ERR_NULL;
-    if (n_blobs < 1) return RPY_ERR_ARG;
-    return matvec_rows(wall != 0, prec, n_blobs, n_rhs, 0, n_blobs, d_pos, d_force, d_vel, a, eta, d_workspace,
-                       workspace_bytes_, cuda_stream, cuda_events4);
 }
 
 size_t rpy_matvec_host_scratch_bytes(rpy_prec prec, int64_t n_blobs, int n_rhs)

@@ -193,7 +193,9 @@ struct PrecondView {
     const int64_t* offsets; const int64_t* mat_off; int* info; double* factors; double* Y; double* Nt;
 };
 __host__ __device__ inline size_t align_up_hd(size_t x) { return (x + 255) / 256 * 256; }
-// header: [0] magic, [1] n_bodies, [2] n_blobs, [3] total_mat (doubles in the factor region)
+// header: [0] magic, [1] n_bodies, [2] n_blobs, [3] total_mat (doubles in the factor region),
+//         [4] first body whose factorisation failed, -1 if none (written by precond_finish_kernel)
+constexpr int kHdrWords = 5;
 __host__ __device__ inline PrecondView view_of(void* base, int64_t nb, int64_t n_blobs, int64_t total_mat)
 {
     unsigned char* b = static_cast<unsigned char*>(base);
@@ -426,13 +428,34 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
     }
     __syncthreads();
     if (tid == 0) {
-        double nt[36];
-        const bool ok = sym6_pinv(s_n, nt);
-        for (int e = 0; e < 36; ++e) Ntg[(size_t)p * 36 + e] = ok ? nt[e] : 0.0;
+        // The 6x6 mixes a force/velocity block (~ eta L), two coupling blocks (~ eta L^2) and a torque/angular
+        // velocity block (~ eta L^3): its spectrum, and with it the cut-off of the pseudo-inverse, would depend
+        // on the unit of length.  Lengths are therefore taken in units of the blob radius first, S' = D S D with
+        // D = diag(1, 1, 1, 1/a, 1/a, 1/a), and the result is scaled back, S^+ := D S'^+ D (reading A18).
+        double sc[36], nt[36];
+        for (int e = 0; e < 36; ++e) sc[e] = s_n[e] * (e / 6 >= 3 ? inv_a : 1.0) * (e % 6 >= 3 ? inv_a : 1.0);
+        const bool ok = sym6_pinv(sc, nt);
+        for (int e = 0; e < 36; ++e)
+            Ntg[(size_t)p * 36 + e] = ok ? nt[e] * (e / 6 >= 3 ? inv_a : 1.0) * (e % 6 >= 3 ? inv_a : 1.0) : 0.0;
         info[p] = ok ? 0 : m + 1;
     }
     if (in_smem)
         for (int e = tid; e < m * m; e += kBuildThreads) G[e] = A[(size_t)(e / m) * ld + e % m];
+}
+
+// After the build: header word 4 = the first body whose info is non-zero (-1: none), so that reading the
+// outcome later is a read-only copy of the header.  One CTA.
+__global__ void precond_finish_kernel(const int* __restrict__ info, int64_t n_bodies, int64_t* __restrict__ hdr)
+{
+    __shared__ long long s_min;
+    if (threadIdx.x == 0) s_min = (long long)1 << 62;
+    __syncthreads();
+    long long mine = (long long)1 << 62;
+    for (int64_t p = threadIdx.x; p < n_bodies; p += blockDim.x)
+        if (info[p] != 0 && p < mine) mine = p;
+    if (mine != ((long long)1 << 62)) atomicMin(&s_min, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) hdr[4] = s_min == ((long long)1 << 62) ? -1 : s_min;
 }
 
 // ------------------------------------------------------------------ preconditioner apply
@@ -452,7 +475,14 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
     in += (int64_t)blockIdx.y * vec_stride; out += (int64_t)blockIdx.y * vec_stride;
     if (lam32) lam32 += (int64_t)blockIdx.y * 3 * n_blobs;
     const int64_t* hdr = static_cast<const int64_t*>(precond);
-    if (p >= n_bodies || hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) return;
+    if (hdr[0] != kMagic || hdr[1] != n_bodies || hdr[2] != n_blobs) {
+        // not a preconditioner of these bodies: fail loudly -- the whole output becomes NaN
+        const int64_t n = 3 * n_blobs + 6 * n_bodies;
+        for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+            out[i] = __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    if (p >= n_bodies) return;
     const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
     const int64_t b0 = pv.offsets[p];
     const int m = 3 * (int)(pv.offsets[p + 1] - b0);
@@ -959,7 +989,7 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
     if (precond_bytes < L.total || ((uintptr_t)d_precond % kAlign) != 0) return RPY_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // tables: header (4 words), the caller's offsets copied up as they are, matrix offsets scanned on the device
-    const int64_t hdr[4] = {kMagic, n_bodies, n_blobs, L.total_mat};
+    const int64_t hdr[kHdrWords] = {kMagic, n_bodies, n_blobs, L.total_mat, -1};
     size_t smem = 0;
     for (int64_t p = 0; p < n_bodies; ++p) {
         const int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]);
@@ -984,6 +1014,8 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
                                                                                    v.factors, v.Y, v.Nt, 1.0 / a, scale);
     }
     RPY_CUDA_TRY(cudaGetLastError());
+    precond_finish_kernel<<<1, 256, 0, st>>>(v.info, n_bodies, reinterpret_cast<int64_t*>(base));
+    RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
 
@@ -991,28 +1023,17 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
 
 namespace {
 
-__global__ void first_bad_kernel(const void* precond, int64_t n_bodies, long long* out)
+// Copies the header down (read-only) and checks that it is a preconditioner of these bodies; *h_first = the
+// first body whose factorisation failed, else -1.  n_blobs < 0: not checked (rpy_rigid_precond_info).
+rpy_status first_bad(int64_t n_bodies, int64_t n_blobs, const void* precond, int64_t* h_first, cudaStream_t st)
 {
-    const int64_t* hdr = static_cast<const int64_t*>(precond);
-    if (hdr[0] != kMagic || hdr[1] != n_bodies) { if (blockIdx.x == 0 && threadIdx.x == 0) *out = -2; return; }
-    const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, hdr[2], hdr[3]);
-    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_bodies; p += (int64_t)gridDim.x * blockDim.x)
-        if (pv.info[p] != 0) atomicMin(out, (long long)p);
-}
-
-// Reads the first failed body through scratch[0] (a device int64 the caller owns).
-rpy_status first_bad(int64_t n_bodies, const void* precond, long long* d_scratch, int64_t* h_first, cudaStream_t st)
-{
-    const long long big = (long long)1 << 62;
-    RPY_CUDA_TRY(cudaMemcpyAsync(d_scratch, &big, 8, cudaMemcpyHostToDevice, st));
-    first_bad_kernel<<<64, 256, 0, st>>>(precond, n_bodies, d_scratch);
-    RPY_CUDA_TRY(cudaGetLastError());
-    long long r = 0;
-    RPY_CUDA_TRY(cudaMemcpyAsync(&r, d_scratch, 8, cudaMemcpyDeviceToHost, st));
+    int64_t hdr[kHdrWords] = {0, 0, 0, 0, 0};
+    RPY_CUDA_TRY(cudaMemcpyAsync(hdr, precond, sizeof hdr, cudaMemcpyDeviceToHost, st));
     RPY_CUDA_TRY(cudaStreamSynchronize(st));
-    if (r == -2) { *h_first = -1; return RPY_ERR_ARG; }          // not a preconditioner of these bodies
-    *h_first = r == big ? -1 : (int64_t)r;
-    return r == big ? RPY_OK : st_of(RPY_ERR_NOT_SPD);
+    *h_first = -1;
+    if (hdr[0] != kMagic || hdr[1] != n_bodies || (n_blobs >= 0 && hdr[2] != n_blobs)) return RPY_ERR_ARG;
+    *h_first = hdr[4];
+    return hdr[4] < 0 ? RPY_OK : st_of(RPY_ERR_NOT_SPD);
 }
 
 }  // namespace
@@ -1023,9 +1044,7 @@ rpy_status rpy_rigid_precond_info(int64_t n_bodies, const void* d_precond, int64
 {
     if (n_bodies < 1) return RPY_ERR_ARG;
     if (!d_precond || !h_first_bad_body) return RPY_ERR_NULL;
-    // header word [0] is the magic; words [1..3] are sizes: the unused tail of the 256-byte header is scratch
-    long long* scratch = reinterpret_cast<long long*>(const_cast<void*>(d_precond)) + 8;
-    return first_bad(n_bodies, d_precond, scratch, h_first_bad_body, static_cast<cudaStream_t>(cuda_stream));
+    return first_bad(n_bodies, -1, d_precond, h_first_bad_body, static_cast<cudaStream_t>(cuda_stream));
 }
 
 rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void* d_precond,
@@ -1125,7 +1144,7 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
     float* const lam32_in_cycle = inner_prec == RPY_PREC_F64 ? nullptr : W.lam32;   // P^-1 also writes float(lambda)
 
     int64_t bad = -1;
-    rpy_status s = first_bad(nb, d_precond, reinterpret_cast<long long*>(W.st.scal), &bad, st);
+    rpy_status s = first_bad(nb, N, d_precond, &bad, st);
     if (s != RPY_OK) return s;
     if (matvec_prec != RPY_PREC_F64) to_float_kernel<<<vgrid(1), 256, 0, st>>>(d_pos, 0, W.pos32, 0, 3 * N);
 

@@ -81,8 +81,11 @@ def gather_velocities(local: torch.Tensor, n_blobs: int, group=None,
 
 
 def reduce_velocities(partial: torch.Tensor, group=None) -> torch.Tensor:
-    """Sum the per-rank PARTIAL velocities of ``rpy_*_matvec_shard`` (full length on every rank) in
-    place with one all-reduce; returns ``partial``, which then holds u on every rank."""
+    """Sum the per-rank PARTIAL velocities of ``rpy_*_matvec_shard`` (full length on every rank, float64
+    on both precision paths so that the cross-rank sum stays an fp64 accumulation) in place with one
+    all-reduce; returns ``partial``, which then holds u on every rank."""
     import torch.distributed as dist
+    if partial.dtype != torch.float64:
+        raise TypeError("reduce_velocities: the partial products of rpy_*_matvec_shard are float64")
     dist.all_reduce(partial, op=dist.ReduceOp.SUM, group=group)
     return partial

@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), f"{n} declared in the header but not exported"
     assert set(names) == set(binding.SIGNATURES), "binding and header disagree on the symbol list"
-    assert lib.rpy_abi_version() == 4
+    assert lib.rpy_abi_version() == 5
 
 
 def test_no_torch_or_oracle_in_native_symbols():
@@ -136,11 +136,9 @@ def test_argument_errors_are_returned_before_any_cuda_work():
     assert rows(F64, 4, 1, 3, 2, p, p, p, 1.0, 1.0, p, 0, None) == 2
     assert rows(F64, 4, 1, 2, 0, p, p, p, 1.0, 1.0, p, 0, None) == 0
     assert lib.rpy_free_matvec_rows(F64, -4, 1, 0, 0, p, p, p, 1.0, 1.0, p, 0, None) == 2
-    # count_below / probe / plan argument checks
+    # count_below / plan argument checks
     assert lib.rpy_wall_count_below(F64, -1, p, 1.0, p, None) == 2
     assert lib.rpy_wall_count_below(F64, 4, p, 1.0, None, None) == 1
-    assert lib.rpy_pipe_peak_probe(9, 10, p, None, None, None) == 2
-    assert lib.rpy_pipe_peak_probe(0, 10, None, None, None, None) == 1
     assert lib.rpy_matvec_launch_plan(F64, 10, 1, 11, None, None, None, None, None) == 2
     assert lib.rpy_last_cuda_error() == 0
 
@@ -175,6 +173,28 @@ def test_product_never_imports_the_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1602_02170_b200 import" not in txt and "import paper_1602_02170_b200" not in txt
+
+
+def test_bench_aids_are_a_library_of_their_own():
+    """The measurement aids (FMA-chain probes, per-kernel events) are not part of the product ABI: they
+    live in bench_aids/ with their own header, build against the product and export what that header declares."""
+    import bench_aids
+    lib = bench_aids.load_library()
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "bench_aids", "rpy_bench_aids.h")).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(rpy_bench_[a-z0-9_]+)\s*\(", hdr)))
+    assert names == ["rpy_bench_coissue_probe", "rpy_bench_matvec_phases", "rpy_bench_pipe_probe"]
+    for n in names:
+        assert hasattr(lib, n)
+    product = binding.load_library()
+    for n in ("rpy_pipe_peak_probe", "rpy_matvec_phases", "rpy_bench_pipe_probe"):
+        assert not hasattr(product, n), f"{n} is a measurement aid and must not be exported by the product"
+    assert "probe" not in open(HEADER).read()
+    # argument checks reach no CUDA call
+    one = ctypes.c_void_p(256)
+    assert lib.rpy_bench_pipe_probe(9, 10, one, None, None, None) == 2
+    assert lib.rpy_bench_pipe_probe(0, 10, None, None, None, None) == 1
+    assert lib.rpy_bench_coissue_probe(9, 10, 10, 0, one, None, None, None, None) == 2
+    assert lib.rpy_bench_matvec_phases(1, 0, 10, 1, one, one, one, 1.0, 1.0, one, 1 << 20, None, None) == 1
 
 
 # ------------------------------------------------------------------ include/rpy_rigid.h

@@ -4,7 +4,9 @@ Tolerances are north_star's: relative L2 error <= 1e-12 for the fp64 path and <=
 fp32 path with fp64 accumulation, over all 3 N k output components (sampled rows at the full
 sizes: the oracle computes each sampled row against ALL sources).  For the fp32 path the oracle
 consumes exactly the values that cross the boundary: the fp32-rounded positions and forces
-promoted to double (reading A8).  The per-blob max error is printed, not gated.
+promoted to double (reading A8).  The per-blob maximum max_i |du_i| / |u_i| is gated too,
+loosely (PB_TOL): a blob whose velocity nearly cancels may lose digits relative to ITS OWN magnitude
+without the method being wrong, but a single wrong row among 10^5 must not hide inside the norm.
 """
 import numpy as np
 import pytest
@@ -16,6 +18,7 @@ from paper_1602_02170_b200 import binding, workloads
 pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-12, "f32": 1e-5}
+PB_TOL = {"f64": 1e-9, "f32": 1e-3}          # per-blob gate (A11)
 DT = {"f64": torch.float64, "f32": torch.float32}
 NP = {"f64": np.float64, "f32": np.float32}
 ORACLE_VARIANT = {"wall": oracle.WALL, "free": oracle.FREE}
@@ -57,6 +60,7 @@ def check(u, ref, prec, what):
     print(f"{what}: prec={prec} rel-L2={e:.3e} per-blob-max={pb:.3e}")
     assert np.isfinite(u).all()
     assert e <= TOL[prec], f"{what}: rel-L2 {e:.3e} > {TOL[prec]}"
+    assert pb <= PB_TOL[prec], f"{what}: per-blob max {pb:.3e} > {PB_TOL[prec]}"
 
 
 # ------------------------------------------------------------------ small cases, every row
@@ -274,16 +278,16 @@ def _full_size(cfg, prec, variant, n_rows):
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_config3_full_size_sampled_rows(prec):
-    _full_size(3, prec, "wall", 256)
+    _full_size(3, prec, "wall", 2048)
 
 
 def test_config4_full_size_sampled_rows():
-    _full_size(4, "f32", "wall", 96)
+    _full_size(4, "f32", "wall", 2048)
 
 
 @pytest.mark.parametrize("variant", ["wall", "free"])
 def test_config5_full_size_sampled_rows(variant):
-    _full_size(5, "f32", variant, 64)
+    _full_size(5, "f32", variant, 2048)
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
