@@ -142,6 +142,3 @@ def matvec_phases(variant: str, pos, force, a: float = 1.0, eta: float = 1.0, *,
         raise RuntimeError(f"rpy_bench_matvec_phases: {binding.rpy_status_string(rc)}")
     return out, events
 
-
-if __name__ == "__main__":
-    print(build(force="--force" in sys.argv))

@@ -18,7 +18,7 @@ from paper_1602_02170_b200 import binding, workloads
 pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-12, "f32": 1e-5}
-PB_TOL = {"f64": 1e-9, "f32": 1e-3}          # per-blob gate (A11)
+PB_TOL = {"f64": 1e-11, "f32": 2e-4}         # per-blob gate (A11); measured maxima: 4e-14 and 3e-5
 DT = {"f64": torch.float64, "f32": torch.float32}
 NP = {"f64": np.float64, "f32": np.float32}
 ORACLE_VARIANT = {"wall": oracle.WALL, "free": oracle.FREE}
