@@ -297,7 +297,7 @@ __global__ void __launch_bounds__(kBuildThreads)
 precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ q,
                      const int64_t* __restrict__ offsets, const int64_t* __restrict__ mat_off,
                      int* __restrict__ info, double* __restrict__ factors, double* __restrict__ Yg,
-                     double* __restrict__ Ntg, double inv_a, double scale)
+                     double* __restrict__ Ntg, double inv_a, double scale, int only_above)
 {
     extern __shared__ __align__(16) double sm[];
     __shared__ double s_n[36];
@@ -307,6 +307,7 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
     const int64_t b0 = offsets[p];
     const int nbp = (int)(offsets[p + 1] - b0);
     const int m = 3 * nbp;
+    if (m <= only_above) return;                               // precond_build_reg_kernel takes this body
     const bool in_smem = m <= kSmemBodyM;
     double* const G = factors + mat_off[p];
     const int ld = in_smem ? (m | 1) : m;
@@ -441,6 +442,282 @@ precond_build_kernel(const double* __restrict__ pos, const double* __restrict__ 
     }
     if (in_smem)
         for (int e = tid; e < m * m; e += kBuildThreads) G[e] = A[(size_t)(e / m) * ld + e % m];
+}
+
+// ------------------------------------------------------------------ preconditioner build, register-resident
+// Bodies with m = 3 n_p <= kRegMaxM (the paper's: 12-42 blobs per body): the matrix never
+// sits in shared memory.  The augmented symmetric matrix
+//     A = [ M^(pp)   K_p ]        (m padded to a multiple of 8 with an identity block; K_p padded to 8 columns)
+//         [ K_p^T    0   ]
+// is cut into 8 x 8 tiles of its lower triangle, ONE TILE PER THREAD, held in 64 double registers for the
+// whole kernel.  The block form of the symmetric sweep operator is applied to the pivot blocks p of M^(pp)
+// (4 rows each) in turn:
+//     P = A_pp^-1,  W = A_{:,p} P,   A <- A - W A_{:,p}^T  everywhere,   then  A_{:,p} = W,  A_pp = -P,
+// the same formula for blocks already swept and blocks still to come, so every thread does the same work
+// in every step and nothing shrinks.  After all pivot blocks of M^(pp):
+//     A = [ -(M^(pp))^-1           (M^(pp))^-1 K_p      ]     i.e. the explicit inverse ("dense matrix
+//         [ K_p^T (M^(pp))^-1     -K_p^T (M^(pp))^-1 K_p ]     inversion"), Y and the 6 x 6
+// Schur complement of Eq. (19) in one pass, m^3/2 fused multiply-adds, the work of Cholesky
+// + triangular inverse + L^-T L^-1.  A step exchanges only the m x 4 panel A_{:,p} and W through shared
+// memory (two barriers, panels double-buffered): each thread loads 2 x 8 doubles per 64 multiply-adds.
+// The pivots of the 4 x 4 blocks are Schur complements of an SPD matrix: a non-positive one reports the body
+// as not positive definite, as the Cholesky factorisation did.
+constexpr int kRT = 8;                         // thread tile
+constexpr int kRegMaxM = 128;                  // largest m = 3 n_p on this path
+constexpr int kRegMaxTA = kRegMaxM / kRT + 1;  // tile rows incl. the K^T row
+constexpr int kRegMaxThreads = 160;            // >= 17 * 18 / 2 = 153 tiles
+constexpr int kPanelStride = 10;               // doubles per 8 panel rows in shared memory (spreads the banks)
+constexpr int kPanelLen = kRegMaxTA * kPanelStride;
+
+__device__ __forceinline__ int panel_at(int row) { return (row >> 3) * kPanelStride + (row & 7); }
+
+// K_p[3 b + comp][c] for the blob at d = r_b - q_p: [I | C_b], C_b = [[0, dz, -dy], [-dz, 0, dx], [dy, -dx, 0]]
+__device__ __forceinline__ double k_entry(int comp, int c, double dx, double dy, double dz)
+{
+    if (c < 3) return comp == c ? 1.0 : 0.0;
+    const int cc = c - 3;
+    if (comp == cc) return 0.0;
+    if (comp == 0) return cc == 1 ? dz : -dy;
+    if (comp == 1) return cc == 0 ? -dz : dx;
+    return cc == 0 ? dy : -dx;
+}
+
+// P = B^-1 for the symmetric positive definite 4 x 4 block B = A[PO..PO+3][PO..PO+3] of a diagonal tile, by four
+// scalar sweeps (all indices compile-time).  Returns false when a pivot is not positive and finite.
+template <int PO>
+__device__ __forceinline__ bool pivot_inverse(const double (&A)[kRT][kRT], double (&P)[4][4])
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) P[i][j] = A[PO + i][PO + j];
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const double d = P[k][k];
+        ok = ok && d > 0.0 && isfinite(d);
+        const double inv = 1.0 / d;
+        double w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w[i] = P[i][k] * inv;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (i != k && j != k) P[i][j] = fma(-w[i], P[k][j], P[i][j]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (i != k) { P[i][k] = w[i]; P[k][i] = w[i]; }
+        P[k][k] = -inv;
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) P[i][j] = -P[i][j];       // the sweeps leave -B^-1
+    return ok;
+}
+
+// One sweep step for pivot rows 8 Pt + PO .. + 3 (PO = 0 or 4, compile-time so that the register tile is only
+// ever indexed with constants).  Cp, Wp: this step's panel buffers [4][kPanelLen]; Pm: its 4 x 4 inverse.
+template <int PO>
+__device__ __forceinline__ void sweep_step(double (&A)[kRT][kRT], bool has_tile, int I, int J, int Pt, int n_rows,
+                                           double* __restrict__ Cp, double* __restrict__ Wp, double* __restrict__ Pm,
+                                           int* s_fail, int step_no)
+{
+    // (a) the panel A_{:,p}: rows of tile row I from the tiles (I, Pt), I >= Pt; rows of tile row J < Pt from the
+    //     transposes of the tiles (Pt, J); the owner of (Pt, Pt) also inverts the pivot block
+    if (has_tile && J == Pt) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int r = 0; r < kRT; ++r) Cp[c * kPanelLen + I * kPanelStride + r] = A[r][PO + c];
+        if (I == Pt) {
+            double P[4][4];
+            if (!pivot_inverse<PO>(A, P)) *s_fail = step_no + 1;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) Pm[4 * i + j] = P[i][j];
+        }
+    } else if (has_tile && I == Pt) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int q = 0; q < kRT; ++q) Cp[c * kPanelLen + J * kPanelStride + q] = A[PO + c][q];
+    }
+    __syncthreads();
+    if (*s_fail) return;                                      // uniform: written before the barrier
+    // (b) W = A_{:,p} P, one row per thread
+    for (int i = threadIdx.x; i < n_rows; i += blockDim.x) {
+        const int at = panel_at(i);
+        const double c0 = Cp[at], c1 = Cp[kPanelLen + at], c2 = Cp[2 * kPanelLen + at], c3 = Cp[3 * kPanelLen + at];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            Wp[j * kPanelLen + at] = fma(c3, Pm[12 + j], fma(c2, Pm[8 + j], fma(c1, Pm[4 + j], c0 * Pm[j])));
+    }
+    __syncthreads();
+    if (!has_tile) return;
+    // (c) A_IJ -= W_I A_{J,p}^T
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+        double w[kRT], cj[kRT];
+        const double2* wp = reinterpret_cast<const double2*>(Wp + c * kPanelLen + I * kPanelStride);
+        const double2* cp = reinterpret_cast<const double2*>(Cp + c * kPanelLen + J * kPanelStride);
+#pragma unroll
+        for (int h = 0; h < kRT / 2; ++h) {
+            const double2 a = wp[h], b = cp[h];
+            w[2 * h] = a.x; w[2 * h + 1] = a.y; cj[2 * h] = b.x; cj[2 * h + 1] = b.y;
+        }
+#pragma unroll
+        for (int r = 0; r < kRT; ++r)
+#pragma unroll
+            for (int q = 0; q < kRT; ++q) A[r][q] = fma(-w[r], cj[q], A[r][q]);
+    }
+    // (d) the pivot rows and columns themselves: A_{:,p} = W, A_{p,:} = W^T, A_pp = -P
+    if (J == Pt) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int r = 0; r < kRT; ++r) A[r][PO + c] = Wp[c * kPanelLen + I * kPanelStride + r];
+    }
+    if (I == Pt) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int q = 0; q < kRT; ++q) A[PO + c][q] = Wp[c * kPanelLen + J * kPanelStride + q];
+        if (J == Pt) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) A[PO + i][PO + j] = -Pm[4 * i + j];
+        }
+    }
+}
+
+template <bool WALL>
+__global__ void __maxnreg__(200)        // 160 threads x 200 registers: two CTAs per SM, no spills
+precond_build_reg_kernel(const double* __restrict__ pos, const double* __restrict__ q,
+                         const int64_t* __restrict__ offsets, const int64_t* __restrict__ mat_off,
+                         int* __restrict__ info, double* __restrict__ factors, double* __restrict__ Yg,
+                         double* __restrict__ Ntg, double inv_a, double scale)
+{
+    __shared__ __align__(16) double s_C[2][4 * kPanelLen];
+    __shared__ __align__(16) double s_W[2][4 * kPanelLen];
+    __shared__ __align__(16) double s_P[2][16];
+    __shared__ int s_fail;
+    const int p = blockIdx.x, tid = threadIdx.x;
+    const int64_t b0 = offsets[p];
+    const int nbp = (int)(offsets[p + 1] - b0);
+    const int m = 3 * nbp;
+    if (m > kRegMaxM) return;                                  // the shared/global-memory kernel takes this body
+    double* const G = factors + mat_off[p];
+    const int T = (m + kRT - 1) / kRT, TA = T + 1;             // tile rows of M^(pp); with the K^T row
+    const int n_tiles = TA * (TA + 1) / 2;
+    if (tid == 0) s_fail = 0;
+
+    // M^(pp) into the body's slot of `factors` (overwritten by the inverse at the end): one pair block per
+    // unordered blob pair, written with its transpose (M_ji = M_ij^T)
+    for (int e = tid; e < nbp * (nbp + 1) / 2; e += blockDim.x) {
+        int bi = (int)((sqrtf(8.0f * (float)e + 1.0f) - 1.0f) * 0.5f);
+        while ((bi + 1) * (bi + 2) / 2 <= e) ++bi;
+        while (bi * (bi + 1) / 2 > e) --bi;
+        const int bj = e - bi * (bi + 1) / 2;
+        const double* ri = pos + 3 * (b0 + bi);
+        const double* rj = pos + 3 * (b0 + bj);
+        double B[9];
+        pair_block<WALL>(ri[0] * inv_a, ri[1] * inv_a, ri[2] * inv_a, rj[0] * inv_a, rj[1] * inv_a, rj[2] * inv_a, B);
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                G[(size_t)(3 * bi + r) * m + 3 * bj + c] = scale * B[3 * r + c];
+                G[(size_t)(3 * bj + c) * m + 3 * bi + r] = scale * B[3 * r + c];
+            }
+    }
+    __syncthreads();
+
+    // this thread's tile (I, J), J <= I, of the augmented matrix
+    const bool has_tile = tid < n_tiles;
+    int I = 0;
+    while ((I + 1) * (I + 2) / 2 <= tid) ++I;
+    const int J = tid - I * (I + 1) / 2;
+    const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
+    double A[kRT][kRT];
+    if (has_tile) {
+#pragma unroll
+        for (int r = 0; r < kRT; ++r)
+#pragma unroll
+            for (int c = 0; c < kRT; ++c) {
+                const int gi = kRT * I + r, gj = kRT * J + c;
+                double v;
+                if (I < T) v = (gi < m && gj < m) ? G[(size_t)gi * m + gj] : (gi == gj ? 1.0 : 0.0);
+                else if (J < T && r < 6 && gj < m) {              // row r of K_p^T
+                    const double* rb = pos + 3 * (b0 + gj / 3);
+                    v = k_entry(gj % 3, r, rb[0] - qx, rb[1] - qy, rb[2] - qz);
+                } else v = 0.0;
+                A[r][c] = v;
+            }
+    }
+    __syncthreads();                                           // everyone has read M^(pp) from G
+
+    const int n_rows = kRT * TA;
+    for (int s = 0; s < 2 * T; ++s) {
+        const int b = s & 1;
+        if (s & 1) sweep_step<4>(A, has_tile, I, J, s >> 1, n_rows, s_C[b], s_W[b], s_P[b], &s_fail, s);
+        else       sweep_step<0>(A, has_tile, I, J, s >> 1, n_rows, s_C[b], s_W[b], s_P[b], &s_fail, s);
+        if (s_fail) break;                                     // uniform (see sweep_step)
+    }
+    if (s_fail) {
+        if (tid == 0) info[p] = s_fail;
+        return;
+    }
+    if (tid == 0) info[p] = 0;
+    if (!has_tile) return;
+    if (I < T) {                                               // (M^(pp))^-1, full symmetric storage
+#pragma unroll
+        for (int r = 0; r < kRT; ++r)
+#pragma unroll
+            for (int c = 0; c < kRT; ++c) {
+                const int gi = kRT * I + r, gj = kRT * J + c;
+                if (gi < m && gj < m && (I != J || c <= r)) {      // a diagonal tile stores its lower half twice:
+                    G[(size_t)gi * m + gj] = -A[r][c];             // the result is symmetric bit for bit
+                    G[(size_t)gj * m + gi] = -A[r][c];
+                }
+            }
+    } else if (J < T) {                                        // Y = (M^(pp))^-1 K_p, [m][6]
+#pragma unroll
+        for (int r = 0; r < 6; ++r)
+#pragma unroll
+            for (int c = 0; c < kRT; ++c) {
+                const int gj = kRT * J + c;
+                if (gj < m) Yg[b0 * 18 + (size_t)gj * 6 + r] = A[r][c];
+            }
+    } else {                                                   // K_p^T (M^(pp))^-1 K_p, inverted by ntilde_kernel
+#pragma unroll
+        for (int r = 0; r < 6; ++r)
+#pragma unroll
+            for (int c = 0; c < 6; ++c) Ntg[(size_t)p * 36 + 6 * r + c] = -A[r][c];
+    }
+}
+
+// N~_pp = (K_p^T (M^(pp))^-1 K_p)^+ in place for the bodies of the register path, one thread per body.
+// The 6x6 mixes a force/velocity block (~ eta L), two coupling blocks (~ eta L^2) and a torque/angular velocity
+// block (~ eta L^3): its spectrum, and with it the cut-off of the pseudo-inverse, would depend on the unit of
+// length.  Lengths are therefore taken in units of the blob radius first, S' = D S D with
+// D = diag(1, 1, 1, 1/a, 1/a, 1/a), and the result is scaled back, S^+ := D S'^+ D (reading A18).
+__global__ void ntilde_kernel(const int64_t* __restrict__ offsets, int* __restrict__ info, double* __restrict__ Ntg,
+                              int64_t n_bodies, double inv_a)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_bodies) return;
+    const int m = 3 * (int)(offsets[p + 1] - offsets[p]);
+    if (m > kRegMaxM || info[p] != 0) return;
+    double sc[36], nt[36];
+    for (int e = 0; e < 36; ++e) sc[e] = Ntg[p * 36 + e] * (e / 6 >= 3 ? inv_a : 1.0) * (e % 6 >= 3 ? inv_a : 1.0);
+    const bool ok = sym6_pinv(sc, nt);
+    for (int e = 0; e < 36; ++e)
+        Ntg[p * 36 + e] = ok ? nt[e] * (e / 6 >= 3 ? inv_a : 1.0) * (e % 6 >= 3 ? inv_a : 1.0) : 0.0;
+    if (!ok) info[p] = m + 1;
 }
 
 // After the build: header word 4 = the first body whose info is non-zero (-1: none), so that reading the
@@ -990,9 +1267,14 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // tables: header (4 words), the caller's offsets copied up as they are, matrix offsets scanned on the device
     const int64_t hdr[kHdrWords] = {kMagic, n_bodies, n_blobs, L.total_mat, -1};
+    // bodies with 3 n_p <= kRegMaxM: the register-resident sweep; larger ones: the shared/global-memory Cholesky
     size_t smem = 0;
+    int max_small = 0;
+    bool any_big = false;
     for (int64_t p = 0; p < n_bodies; ++p) {
         const int64_t m = 3 * (h_offsets[p + 1] - h_offsets[p]);
+        if (m <= kRegMaxM) { if (m > max_small) max_small = (int)m; continue; }
+        any_big = true;
         if (m <= kSmemBodyM) { size_t need = ((size_t)(m | 1) * m + 6 * m) * 8; if (need > smem) smem = need; }
     }
     unsigned char* base = static_cast<unsigned char*>(d_precond);
@@ -1004,14 +1286,28 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
     PrecondView v = view_of(d_precond, n_bodies, n_blobs, L.total_mat);
     const double PI = 3.14159265358979323846;
     const double scale = 1.0 / (6.0 * PI * eta * a);
-    if (wall) {
-        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        precond_build_kernel<true><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
-                                                                                  v.factors, v.Y, v.Nt, 1.0 / a, scale);
-    } else {
-        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        precond_build_kernel<false><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
-                                                                                   v.factors, v.Y, v.Nt, 1.0 / a, scale);
+    if (max_small > 0) {
+        const int TA = (max_small + kRT - 1) / kRT + 1;
+        const int threads = (TA * (TA + 1) / 2 + 31) / 32 * 32;
+        if (wall) precond_build_reg_kernel<true><<<(unsigned)n_bodies, threads, 0, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                       v.factors, v.Y, v.Nt, 1.0 / a, scale);
+        else      precond_build_reg_kernel<false><<<(unsigned)n_bodies, threads, 0, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                        v.factors, v.Y, v.Nt, 1.0 / a, scale);
+        RPY_CUDA_TRY(cudaGetLastError());
+        ntilde_kernel<<<(unsigned)((n_bodies + 127) / 128), 128, 0, st>>>(v.offsets, v.info, v.Nt, n_bodies, 1.0 / a);
+        RPY_CUDA_TRY(cudaGetLastError());
+    }
+    if (any_big) {
+        const int only_above = max_small > 0 ? kRegMaxM : 0;
+        if (wall) {
+            RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            precond_build_kernel<true><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                      v.factors, v.Y, v.Nt, 1.0 / a, scale, only_above);
+        } else {
+            RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            precond_build_kernel<false><<<(unsigned)n_bodies, kBuildThreads, smem, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
+                                                                                       v.factors, v.Y, v.Nt, 1.0 / a, scale, only_above);
+        }
     }
     RPY_CUDA_TRY(cudaGetLastError());
     precond_finish_kernel<<<1, 256, 0, st>>>(v.info, n_bodies, reinterpret_cast<int64_t*>(base));
