@@ -367,7 +367,8 @@ def time_solve(torch, cfg: int, matvec_prec: str, tol: float, restart: int = 60)
         e1.record(); torch.cuda.synchronize()
         return e0.elapsed_time(e1) / reps, out
 
-    build_ms, pc = timed(lambda: rigid.rpy_rigid_precond_build(b, "wall", wl.a, wl.eta, check=False), reps=2)
+    pbuf = torch.empty(rigid.rpy_rigid_precond_bytes(hb.offsets), dtype=torch.uint8, device=dev)
+    build_ms, pc = timed(lambda: rigid.rpy_rigid_precond_build(b, "wall", wl.a, wl.eta, check=False, buf=pbuf), reps=5)
     rigid.rpy_rigid_precond_info(pc)
     vec = torch.randn(b.n, dtype=torch.float64, device=dev)
     out = torch.empty_like(vec)

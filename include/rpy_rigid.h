@@ -56,7 +56,7 @@ extern "C" {
  * fp64 product for the residual each cycle starts from.  "Krylov methods ... allow one to lower the
  * accuracy of the matrix-vector product as the residual is reduced": a cycle ends
  * when its fp32 residual estimate has dropped by 1e-4 (or reached tol), x is updated, the true fp64
- * residual of Eq. (11) is recomputed and decides convergence.  Reaches fp64 tolerances at mostly
+ * residual of Eq. (11) is recomputed and decides convergence (tol = 1e-8: two cycles, two fp64 products).  Reaches fp64 tolerances at mostly
  * fp32 cost; *h_rel_resid is then the TRUE relative residual. */
 #define RPY_PREC_MIXED 2
 
@@ -117,32 +117,60 @@ rpy_status rpy_rigid_precond_get(int64_t n_bodies, const int64_t *h_offsets, con
 rpy_status rpy_rigid_blob_positions(rpy_prec prec, int64_t n_bodies, int blobs_per_body, const void *d_template,
                                     const void *d_centres, const void *d_quats, void *d_pos, void *cuda_stream);
 
-/* Workspace of the solve: restart+1 Krylov vectors, three work vectors, the matvec workspace and
- * (fp32 matvec) float copies of positions, iterate and product.                                   */
+/* Workspace of the solve: restart+1 Krylov vectors, four work vectors, the matvec workspace (of the fp64
+ * product too when matvec_prec is not RPY_PREC_F64: such solves form fp64 residuals) and, for fp32 products,
+ * float copies of positions, iterate and product.                                                  */
 size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int restart);
+
+/* Optional extras of the solve (pass NULL for none).  The library creates no CUDA object of its own:
+ *   side_stream, side_event   a second cudaStream_t and a cudaEvent_t (timing may be disabled) of the
+ *       caller.  With them the host reads the outcome of iteration j on side_stream, ordered after that
+ *       iteration by side_event, while `cuda_stream` already runs iteration j+1; without them it reads on
+ *       `cuda_stream` and the device idles while the next iteration is being enqueued.
+ *   shard, n_shards, reduce, reduce_ctx   multi-GPU (one process per GPU, all arguments replicated): rank
+ *       `shard` of `n_shards` computes its share of every product M lambda (rpy_*_matvec_shard's unordered
+ *       tile pairs) and calls reduce(reduce_ctx, d_buf, count, cuda_stream) once per product; the hook must
+ *       make d_buf[0..count) (doubles, device) the SUM over all ranks, in stream order on cuda_stream (e.g.
+ *       an in-place NCCL all-reduce), and return 0.  Everything else of the iteration is replicated, so the
+ *       ranks take the same decisions.  n_shards > 1 needs n_rhs == 1 and n_blobs >= 3,584.              */
+typedef int (*rpy_reduce_fn)(void *reduce_ctx, double *d_buf, int64_t count, void *cuda_stream);
+typedef struct rpy_rigid_solve_ext {
+    void *side_stream;
+    void *side_event;
+    int shard;
+    int n_shards;               /* 0 or 1: the whole product on this GPU */
+    rpy_reduce_fn reduce;
+    void *reduce_ctx;
+} rpy_rigid_solve_ext;
 
 /* Solves the mobility problem, Eq. (11), for lambda and U given the applied forces/torques F and an
  * optional slip velocity, by right-preconditioned GMRES(restart) from a zero initial guess: the
  * iteration stops when the residual of (11) is <= tol * ||[slip; -F]|| (Table III: tol = 1e-8,
  * PAPER.md:680) or after max_iter matrix applications.  One iteration = P^-1 (above), the O(N^2)
  * product M lambda (rpy_wall_matvec / rpy_free_matvec with matvec_prec), K, K^T, classical
- * Gram-Schmidt applied twice, and a Givens update of the small Hessenberg problem -- all on the
- * device; the host reads one double (the residual norm) per iteration, so the call SYNCHRONISES.
- * That read-back runs on a second stream created (and destroyed) inside the call, while `cuda_stream`
- * already applies the preconditioner of the next iteration: the only CUDA objects the library creates.
+ * Gram-Schmidt applied twice, a Givens update of the small Hessenberg problem and the stopping test --
+ * all on the device (seven launches).  The host reads 80 bytes per iteration to follow the device's
+ * decision and to fill h_history, so the call SYNCHRONISES; see rpy_rigid_solve_ext for how that read
+ * is kept off the critical path.
  *   wall        != 0: wall-corrected M in the product (the preconditioner is whatever was built)
+ *   matvec_prec RPY_PREC_F64; RPY_PREC_F32_ACC64 (fp32 products; converges on the fp32 operator's residual
+ *               estimate, then ONE fp64 product gives the true residual that is reported); RPY_PREC_MIXED
  *   d_F         [n_bodies][6] device;  d_slip [n_blobs][3] device or NULL (zero slip)
  *   d_lambda    [n_blobs][3], d_U [n_bodies][6] : device, overwritten
  *   h_history   host, max_iter+1 doubles or NULL: relative residual after each iteration, [0] = 1
- *   h_n_iter    host, matrix applications used;  h_rel_resid host, final relative residual estimate
- * Returns RPY_OK also when max_iter was reached without convergence (check *h_rel_resid).         */
+ *   h_n_iter    host, matrix applications used;  h_rel_resid host, final relative residual: the true
+ *               residual of Eq. (11) (fp64 product) unless matvec_prec is RPY_PREC_F64, where the Arnoldi
+ *               estimate IS the residual of the operator used
+ * Returns RPY_OK also when max_iter was reached without convergence (check *h_rel_resid).
+ * A d_precond that was not built for these bodies (n_bodies, n_blobs) is RPY_ERR_ARG.                */
 rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
                                     const double *d_pos, const double *d_q, const int64_t *d_offsets,
                                     const double *d_F, const double *d_slip, double a, double eta,
                                     const void *d_precond, double tol, int restart, int max_iter,
                                     double *d_lambda, double *d_U,
                                     double *h_history, int *h_n_iter, double *h_rel_resid,
-                                    void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+                                    void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                                    const rpy_rigid_solve_ext *ext);
 
 /* The same for n_rhs (1..RPY_RIGID_MAX_BATCH) right-hand sides at once -- e.g. the columns of the body
  * mobility matrix N of Eq. (12), one unit force or torque each.  n_rhs independent GMRES processes
@@ -161,7 +189,8 @@ rpy_status rpy_rigid_mobility_solve_batch(int wall, rpy_prec matvec_prec, int64_
                                           const void *d_precond, double tol, int restart, int max_iter,
                                           double *d_lambda, double *d_U,
                                           double *h_history, int *h_n_iter, double *h_rel_resid,
-                                          void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+                                          void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                                          const rpy_rigid_solve_ext *ext);
 
 /* The operator of Eq. (11) alone: out = [M lambda - K U ; -K^T lambda] for a solver vector
  * in = [lambda; U] (tests; residual checks).  d_workspace as for the solve with restart = 1.      */

@@ -34,10 +34,12 @@ __global__ void prepack_kernel(const typename L::S* __restrict__ pos,
                                const typename L::S* __restrict__ force,   // [K][n][3] of this RHS group
                                typename L::S* __restrict__ rec,
                                int64_t n_blobs, int64_t n_padded, int64_t force_rhs_stride,
-                               double inv_a, double* __restrict__ zero, int64_t zero_count)
+                               double inv_a, double* __restrict__ zero, int64_t zero_count,
+                               const int* __restrict__ skip)
 {
     using S = typename L::S;
     using R = RecLayout<L, K>;
+    if (skip != nullptr && *skip != 0) return;      // a caller that enqueues ahead of a device-side decision (rpy_rigid.cu)
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_padded) return;
     // the symmetric kernel's atomic accumulator (3 doubles per blob) is cleared here: one launch less
@@ -126,7 +128,8 @@ template <class L, int K, bool WALL, int T, int BLOCK, int TILE_G, int FLUSH_G, 
 __global__ void __launch_bounds__(BLOCK, MINB)
 allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __restrict__ trec,
                 double* __restrict__ partial,
-                int64_t row_begin, int64_t row_count, int64_t n_tiles, int tiles_per_chunk)
+                int64_t row_begin, int64_t row_count, int64_t n_tiles, int tiles_per_chunk,
+                const int* __restrict__ skip)
 {
     using V = typename L::V;
     using S = typename L::S;
@@ -135,6 +138,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
     static_assert(TILE_G % FLUSH_G == 0, "flush period must divide the tile");
+    if (skip != nullptr && *skip != 0) return;
     static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -302,7 +306,8 @@ template <> __device__ __forceinline__ double lane_elem<float2>(float2 v, int w)
 template <class L, bool WALL, int T, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial, double* __restrict__ gacc,
-                    int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end)
+                    int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end,
+                    const int* __restrict__ skip)
 {
     using V = typename L::V;
     using S = typename L::S;
@@ -310,6 +315,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     constexpr int W = L::W;
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr int TS = BLOCK * T;                  // blobs per tile
+    if (skip != nullptr && *skip != 0) return;
     constexpr int TILE_G = TS / W;                 // records per tile
     constexpr int NSUB = TILE_G / 32;              // sub-tiles of 32 records
     constexpr int NWARP = BLOCK / 32;
@@ -468,10 +474,11 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
 template <class S>
 __global__ void finalise_kernel(const double* __restrict__ partial, S* __restrict__ vel,
                                 int64_t per_chunk /* = K*row_count*3 */, int n_chunks,
-                                int64_t row_count3, int64_t vel_rhs_stride, double scale)
+                                int64_t row_count3, int64_t vel_rhs_stride, double scale,
+                                const int* __restrict__ skip)
 {
     int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= per_chunk) return;
+    if (e >= per_chunk || (skip != nullptr && *skip != 0)) return;
     // four interleaved running sums (fixed assignment chunk -> sum, fixed final order): the loads of
     // different chunks do not wait on one another
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;

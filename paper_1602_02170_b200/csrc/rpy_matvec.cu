@@ -171,10 +171,10 @@ template <class L, int K> constexpr size_t allpairs_smem() { return 2 * (size_t)
 
 template <class L, int K, bool WALL, int T>
 cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typename L::S* trec, double* partial,
-                            int64_t row_begin, int64_t rows, cudaStream_t st)
+                            int64_t row_begin, int64_t rows, cudaStream_t st, const int* skip)
 {
     dim3 grid((unsigned)p.n_target_tiles, (unsigned)p.n_chunks);
-    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, trec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk);
+    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, trec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk, skip);
     return cudaGetLastError();
 }
 
@@ -185,6 +185,16 @@ struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_
 #define RPY_SYM_SMALL_BELOW 50000      // below this many blobs the symmetric kernel runs with 128-blob tiles (measured crossover)
 #endif
 struct Shard { int index; int count; };        // {0, 1}: the whole product
+
+// What varies between the entry points that share run_group.
+struct Opts {
+    Shard sh{0, 1};
+    int64_t vel_stride3 = -1;       // elements between right-hand sides of vel (-1: 3 rows)
+    int64_t force_stride3 = -1;     // the same for force (-1: 3 n)
+    bool vel_f64 = false;           // vel is double whatever the path (partial products of a shard)
+    const int* skip = nullptr;      // device flag: non-zero turns every kernel of the call into a no-op
+    rpy::PartialSums* partials = nullptr;   // non-null: finalise is left to the caller, who gets the slices
+};
 
 inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
 {
@@ -218,19 +228,19 @@ template <> struct SymShape<rpy::Lane<double>> { static constexpr int MINB = RPY
 
 template <class L>
 cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, double* partial, double* gacc,
-                       int64_t n, cudaStream_t st)
+                       int64_t n, cudaStream_t st, const int* skip)
 {
     constexpr int MINB = SymShape<L>::MINB;
     dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
     if (p.tile == kSymTile) {
         size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
-        if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
-        else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+        if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+        else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
     } else {
         constexpr int B2 = kBlock / 2;
         size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
-        if (wall) rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
-        else      rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end);
+        if (wall) rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+        else      rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
     }
     return cudaGetLastError();
 }
@@ -240,10 +250,12 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
                       const typename L::S* pos, const typename L::S* force, void* vel,
                       double a, double eta, unsigned char* ws, cudaStream_t st, void* const* ev,
                       const typename L::S* tpos /* targets of the rectangular product, else nullptr */,
-                      Shard sh, int64_t vel_stride3 /* elements between right-hand sides of vel */,
-                      int64_t force_stride3 /* the same for force */,
-                      bool vel_f64 /* vel is double whatever the path (partial products of a shard) */)
+                      const Opts& o)
 {
+    const Shard sh = o.sh;
+    const int64_t vel_stride3 = o.vel_stride3, force_stride3 = o.force_stride3;
+    const bool vel_f64 = o.vel_f64;
+    const int* skip = o.skip;
     using S = typename L::S;
     S* rec = reinterpret_cast<S*>(ws);
     rpy_prec prec = sizeof(S) == 8 ? RPY_PREC_F64 : RPY_PREC_F32_ACC64;
@@ -271,21 +283,21 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
         rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, n_padded,
-                                                                      force_stride3, 1.0 / a, gacc, sym ? n * 3 : 0);
+                                                                      force_stride3, 1.0 / a, gacc, sym ? n * 3 : 0, skip);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     if (sym) {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
-        if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, partial, gacc, n, st);
+        if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, partial, gacc, n, st, skip);
         else e = cudaErrorInvalidValue;
         n_slices = sp.n_chunks + 1;
     } else {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
         constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
-        if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, trec, partial, row_begin, rows, st)
-                               : launch_allpairs<L, K, true, 1>(p, rec, trec, partial, row_begin, rows, st);
-        else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, trec, partial, row_begin, rows, st)
-                               : launch_allpairs<L, K, false, 1>(p, rec, trec, partial, row_begin, rows, st);
+        if (wall) e = p.T == 2 ? launch_allpairs<L, K, true, T2>(p, rec, trec, partial, row_begin, rows, st, skip)
+                               : launch_allpairs<L, K, true, 1>(p, rec, trec, partial, row_begin, rows, st, skip);
+        else      e = p.T == 2 ? launch_allpairs<L, K, false, T2>(p, rec, trec, partial, row_begin, rows, st, skip)
+                               : launch_allpairs<L, K, false, 1>(p, rec, trec, partial, row_begin, rows, st, skip);
     }
     if (e != cudaSuccess) return e;
     if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[2]), st)) != cudaSuccess) return e;
@@ -295,10 +307,16 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         int64_t blocks = (per_chunk + threads - 1) / threads;
         const double PI = 3.14159265358979323846;
         const double scale = 1.0 / (6.0 * PI * eta * a);
+        if (o.partials) {                           // the caller adds the slices itself (fused into its next kernel)
+            o.partials->partial = partial; o.partials->n_slices = n_slices;
+            o.partials->per_chunk = per_chunk; o.partials->scale = scale;
+            return cudaSuccess;
+        }
+        (void)vel_stride3;
         if (vel_f64) rpy::finalise_kernel<double><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<double*>(vel), per_chunk, n_slices,
-                                                                                     rows * 3, vel_stride3, scale);
+                                                                                     rows * 3, vel_stride3, scale, skip);
         else         rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<S*>(vel), per_chunk, n_slices,
-                                                                               rows * 3, vel_stride3, scale);
+                                                                               rows * 3, vel_stride3, scale, skip);
         e = cudaGetLastError();
     }
     return e;
@@ -308,28 +326,28 @@ template <class L>
 cudaError_t run_all_groups(bool wall, int64_t n, int n_rhs, int64_t row_begin, int64_t rows,
                            const void* d_pos, const void* d_force, void* d_vel,
                            double a, double eta, void* ws, cudaStream_t st, void* const* ev,
-                           const void* d_tpos = nullptr, Shard sh = Shard{0, 1}, int64_t vel_stride3 = -1,
-                           int64_t force_stride3 = -1, bool vel_f64 = false)
+                           const void* d_tpos = nullptr, Opts o = Opts{})
 {
     using S = typename L::S;
     cudaError_t ee;
     if (ev && (ee = cudaEventRecord(static_cast<cudaEvent_t>(ev[0]), st)) != cudaSuccess) return ee;
     const S* pos = static_cast<const S*>(d_pos);
     const S* tp = static_cast<const S*>(d_tpos);
-    if (vel_stride3 < 0) vel_stride3 = rows * 3;
-    if (force_stride3 < 0) force_stride3 = n * 3;
+    if (o.vel_stride3 < 0) o.vel_stride3 = rows * 3;
+    if (o.force_stride3 < 0) o.force_stride3 = n * 3;
     int done = 0;
     while (done < n_rhs) {
         int K = group_k(n_rhs - done);
-        const S* force = static_cast<const S*>(d_force) + (int64_t)done * force_stride3;
-        void* vel = static_cast<unsigned char*>(d_vel) + (size_t)done * vel_stride3 * (vel_f64 ? sizeof(double) : sizeof(S));
+        const S* force = static_cast<const S*>(d_force) + (int64_t)done * o.force_stride3;
+        void* vel = d_vel ? static_cast<unsigned char*>(d_vel) + (size_t)done * o.vel_stride3 * (o.vel_f64 ? sizeof(double) : sizeof(S)) : nullptr;
         unsigned char* w = static_cast<unsigned char*>(ws);
+        void* const* ev1 = done == 0 ? ev : nullptr;
         cudaError_t e;
         switch (K) {
-            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
-            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
-            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
-            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, done == 0 ? ev : nullptr, tp, sh, vel_stride3, force_stride3, vel_f64); break;
+            case 8: e = run_group<L, 8>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, ev1, tp, o); break;
+            case 4: e = run_group<L, 4>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, ev1, tp, o); break;
+            case 2: e = run_group<L, 2>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, ev1, tp, o); break;
+            default: e = run_group<L, 1>(wall, n, row_begin, rows, pos, force, vel, a, eta, w, st, ev1, tp, o); break;
         }
         if (e != cudaSuccess) return e;
         done += K;
@@ -386,10 +404,10 @@ rpy_status matvec_shard(bool wall, rpy_prec prec, int64_t n, int n_rhs, int shar
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaError_t e;
     if (n_rhs == 1 && use_symmetric(n, 1, 0, n)) {
-        const Shard sh{shard, n_shards};
+        Opts o; o.sh = Shard{shard, n_shards}; o.vel_f64 = true;
         e = prec == RPY_PREC_F64
-            ? run_all_groups<rpy::Lane<double>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh, -1, -1, true)
-            : run_all_groups<rpy::Lane<float2>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, sh, -1, -1, true);
+            ? run_all_groups<rpy::Lane<double>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, 1, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o);
     } else {
         const int64_t r0 = n * shard / n_shards, r1 = n * (shard + 1) / n_shards;
         if ((e = cudaMemsetAsync(d_vel, 0, vel_b, st)) != cudaSuccess) return cuda_fail(e);
@@ -397,9 +415,10 @@ rpy_status matvec_shard(bool wall, rpy_prec prec, int64_t n, int n_rhs, int shar
         void* out = static_cast<unsigned char*>(d_vel) + (size_t)r0 * 3 * sizeof(double);
         // rows r0..r1-1 by the plain kernel (never the symmetric one: row_begin/rows are not the whole range,
         // or n is below the symmetric threshold), written in place of the full-length layout
+        Opts o; o.vel_stride3 = n * 3; o.vel_f64 = true;
         e = prec == RPY_PREC_F64
-            ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3, -1, true)
-            : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, n * 3, -1, true);
+            ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, o)
+            : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, r0, r1 - r0, d_pos, d_force, out, a, eta, ws, st, nullptr, nullptr, o);
     }
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
@@ -493,18 +512,29 @@ rpy_status matvec_phases(bool wall, rpy_prec prec, int64_t n_blobs, int n_rhs, c
 
 rpy_status matvec_strided(bool wall, rpy_prec prec, int64_t n, int n_rhs, const void* d_pos, const void* d_force,
                           int64_t force_stride3, void* d_vel, int64_t vel_stride3, double a, double eta,
-                          void* ws, size_t ws_bytes, cudaStream_t st)
+                          void* ws, size_t ws_bytes, cudaStream_t st, const int* d_skip, PartialSums* partials,
+                          int shard, int n_shards, bool vel_f64)
 {
     if (prec != RPY_PREC_F64 && prec != RPY_PREC_F32_ACC64) return RPY_ERR_ARG;
-    if (n < 1 || n > RPY_MAX_BLOBS || n_rhs < 1 || force_stride3 < 3 * n || vel_stride3 < 3 * n) return RPY_ERR_ARG;
-    if (!d_pos || !d_force || !d_vel || !ws) return RPY_ERR_NULL;
+    if (n < 1 || n > RPY_MAX_BLOBS || n_rhs < 1 || force_stride3 < 3 * n) return RPY_ERR_ARG;
+    if (n_shards < 1 || shard < 0 || shard >= n_shards) return RPY_ERR_ARG;
+    if (partials) {                               // one right-hand-side group, so that its slices outlive the call
+        if (n_rhs != group_k(n_rhs)) return RPY_ERR_ARG;
+    } else if (!d_vel || vel_stride3 < 3 * n) return RPY_ERR_ARG;
+    if (n_shards > 1 && !(n_rhs == 1 && use_symmetric(n, 1, 0, n))) return RPY_ERR_ARG;   // shards of the symmetric kernel only
+    if (!d_pos || !d_force || !ws) return RPY_ERR_NULL;
     if (ws_bytes < workspace_bytes(prec, n, n_rhs) || ((uintptr_t)ws % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    Opts o;
+    o.vel_stride3 = partials ? 3 * n : vel_stride3; o.force_stride3 = force_stride3;
+    o.skip = d_skip; o.partials = partials; o.sh = Shard{shard, n_shards}; o.vel_f64 = vel_f64;
     cudaError_t e = prec == RPY_PREC_F64
-        ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, vel_stride3, force_stride3)
-        : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, Shard{0, 1}, vel_stride3, force_stride3);
+        ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o)
+        : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o);
     if (e != cudaSuccess) return cuda_fail(e);
     return RPY_OK;
 }
+
+bool matvec_shardable(int64_t n) { return use_symmetric(n, 1, 0, n); }
 }  // namespace rpy
 
 extern "C" {

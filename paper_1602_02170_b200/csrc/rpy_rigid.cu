@@ -24,6 +24,10 @@ constexpr size_t kAlign = 256;
 constexpr int kSmemBodyM = 162;            // largest 3*blobs whose matrix is factorised in shared memory
 constexpr int kBuildThreads = 256;
 constexpr int64_t kMagic = 0x52505952494744LL;   // "RPYRIGD"
+constexpr int kVecBlocks = 296;            // CTAs of the Krylov vector kernels: 2 per SM
+constexpr int kVecThreads = 256;
+constexpr int kScal = 8;                   // doubles of scalar state per right-hand side of the solve
+constexpr int kSnapBytes = 128;            // one snapshot of the solve's state for the host (16 + 8 * RPY_RIGID_MAX_BATCH <= 128)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline rpy_status st_of(int s) { return static_cast<rpy_status>(s); }
@@ -94,29 +98,64 @@ __global__ void kt_apply_kernel(const double* __restrict__ pos, const double* __
     }
 }
 
+// scale * (sum of the product's per-slice partial sums) for output element e of right-hand side blockIdx.y, the
+// slices added in the order of the product's own finalise kernel (four interleaved running sums).
+__device__ __forceinline__ double sum_slices(const rpy::PartialSums& ps, int64_t e)
+{
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int c = 0;
+    for (; c + 4 <= ps.n_slices; c += 4) {
+        s0 += ps.partial[(int64_t)c * ps.per_chunk + e];
+        s1 += ps.partial[(int64_t)(c + 1) * ps.per_chunk + e];
+        s2 += ps.partial[(int64_t)(c + 2) * ps.per_chunk + e];
+        s3 += ps.partial[(int64_t)(c + 3) * ps.per_chunk + e];
+    }
+    for (; c < ps.n_slices; ++c) s0 += ps.partial[(int64_t)c * ps.per_chunk + e];
+    return ((s0 + s1) + (s2 + s3)) * ps.scale;
+}
+
 // The two O(N) pieces of Eq. (11)'s operator in one pass, one warp per body (blockIdx.y = right-hand side):
-//   out_top[i]  = (vel32 ? double(vel32[i]) : out_top[i]) - (K U)_i        (M lambda is already in place)
+//   out_top[i]  = (M lambda)_i - (K U)_i
 //   out_bot[p]  = -(K^T lambda)_p
-// in = [lambda; U], out = [top; bottom], both with `stride` doubles between right-hand sides.
+// in = [lambda; U], out = [top; bottom], both with `stride` doubles between right-hand sides.  M lambda comes
+// from the product's per-slice partial sums when ps.partial is set (the product's finalise step fused in here:
+// one launch less per iteration, and the fp32 path's result is not rounded to float on the way), else from
+// vel32 (float), else it is already in out_top.
 __global__ void saddle_tail_kernel(const double* __restrict__ pos, const double* __restrict__ q,
                                    const int64_t* __restrict__ offsets, const double* __restrict__ in,
                                    const float* __restrict__ vel32, double* __restrict__ out,
-                                   int64_t n_blobs, int64_t n_bodies, int64_t stride)
+                                   int64_t n_blobs, int64_t n_bodies, int64_t stride, rpy::PartialSums ps,
+                                   const int* __restrict__ skip)
 {
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    if (p >= n_bodies) return;
+    if (skip != nullptr && *skip != 0) return;
     in += (int64_t)blockIdx.y * stride; out += (int64_t)blockIdx.y * stride;
     if (vel32) vel32 += (int64_t)blockIdx.y * 3 * n_blobs;
+    if (ps.partial) {
+        // the bodies of this CTA own a contiguous range of output elements: all threads add the slices for it
+        // (one element per thread and pass, coalesced in every slice), then each warp goes on with its body
+        const int64_t pA = (int64_t)blockIdx.x * (blockDim.x >> 5);
+        const int64_t pB = pA + (blockDim.x >> 5) < n_bodies ? pA + (blockDim.x >> 5) : n_bodies;
+        if (pA < n_bodies) {
+            const int64_t e1 = 3 * offsets[pB], base = (int64_t)blockIdx.y * n_blobs * 3;
+            for (int64_t e = 3 * offsets[pA] + threadIdx.x; e < e1; e += blockDim.x) out[e] = sum_slices(ps, base + e);
+        }
+        __syncthreads();
+    }
+    if (p >= n_bodies) return;
     const double* U = in + 3 * n_blobs + 6 * p;
     const double ux = U[0], uy = U[1], uz = U[2], wx = U[3], wy = U[4], wz = U[5];
     const double qx = q[3 * p + 0], qy = q[3 * p + 1], qz = q[3 * p + 2];
     double s[6] = {0, 0, 0, 0, 0, 0};
     for (int64_t i = offsets[p] + lane; i < offsets[p + 1]; i += 32) {
         const double dx = pos[3 * i + 0] - qx, dy = pos[3 * i + 1] - qy, dz = pos[3 * i + 2] - qz;
-        const double m0 = vel32 ? (double)vel32[3 * i + 0] : out[3 * i + 0];
-        const double m1 = vel32 ? (double)vel32[3 * i + 1] : out[3 * i + 1];
-        const double m2 = vel32 ? (double)vel32[3 * i + 2] : out[3 * i + 2];
+        double m0, m1, m2;
+        if (vel32) {
+            m0 = (double)vel32[3 * i + 0]; m1 = (double)vel32[3 * i + 1]; m2 = (double)vel32[3 * i + 2];
+        } else {
+            m0 = out[3 * i + 0]; m1 = out[3 * i + 1]; m2 = out[3 * i + 2];
+        }
         out[3 * i + 0] = m0 - (ux + (wy * dz - wz * dy));
         out[3 * i + 1] = m1 - (uy + (wz * dx - wx * dz));
         out[3 * i + 2] = m2 - (uz + (wx * dy - wy * dx));
@@ -242,44 +281,68 @@ __device__ __forceinline__ void pair_block(double xi, double yi, double zi, doub
 // about its axis: that direction gets zero mobility), a negative or non-finite spectrum fails.
 __device__ bool sym6_pinv(const double* __restrict__ a_in, double* __restrict__ out)
 {
+    // every index below is a compile-time constant after unrolling: both matrices live in registers
     double a[6][6], v[6][6];
+#pragma unroll
     for (int r = 0; r < 6; ++r)
+#pragma unroll
         for (int c = 0; c < 6; ++c) { a[r][c] = 0.5 * (a_in[6 * r + c] + a_in[6 * c + r]); v[r][c] = r == c ? 1.0 : 0.0; }
+#pragma unroll 1
     for (int sweep = 0; sweep < 30; ++sweep) {
         double off = 0.0, diag = 0.0;
+#pragma unroll
         for (int r = 0; r < 6; ++r)
+#pragma unroll
             for (int c = 0; c < 6; ++c) { if (r != c) off += a[r][c] * a[r][c]; else diag += a[r][c] * a[r][c]; }
         if (!(off > 1e-60 * diag) || !isfinite(off)) break;
+#pragma unroll
         for (int p = 0; p < 5; ++p)
+#pragma unroll
             for (int q = p + 1; q < 6; ++q) {
-                if (a[p][q] == 0.0) continue;
-                const double theta = (a[q][q] - a[p][p]) / (2.0 * a[p][q]);
-                const double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
-                const double c = 1.0 / sqrt(t * t + 1.0), sn = t * c;
-                const double app = a[p][p], aqq = a[q][q], apq = a[p][q];
-                for (int k = 0; k < 6; ++k) {                  // rows / columns p and q of J^T A J, k != p, q
-                    if (k == p || k == q) continue;
-                    const double akp = a[k][p], akq = a[k][q];
-                    a[k][p] = a[p][k] = c * akp - sn * akq;
-                    a[k][q] = a[q][k] = sn * akp + c * akq;
-                }
-                a[p][p] = c * c * app - 2.0 * c * sn * apq + sn * sn * aqq;
-                a[q][q] = sn * sn * app + 2.0 * c * sn * apq + c * c * aqq;
-                a[p][q] = a[q][p] = 0.0;
-                for (int k = 0; k < 6; ++k) {                  // V <- V J
-                    const double vkp = v[k][p], vkq = v[k][q];
-                    v[k][p] = c * vkp - sn * vkq; v[k][q] = sn * vkp + c * vkq;
+                if (a[p][q] != 0.0) {
+                    const double theta = (a[q][q] - a[p][p]) / (2.0 * a[p][q]);
+                    const double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                    const double c = rsqrt(t * t + 1.0), sn = t * c;
+                    const double app = a[p][p], aqq = a[q][q], apq = a[p][q];
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {              // rows / columns p and q of J^T A J, k != p, q
+                        if (k != p && k != q) {
+                            const double akp = a[k][p], akq = a[k][q];
+                            a[k][p] = a[p][k] = c * akp - sn * akq;
+                            a[k][q] = a[q][k] = sn * akp + c * akq;
+                        }
+                    }
+                    a[p][p] = c * c * app - 2.0 * c * sn * apq + sn * sn * aqq;
+                    a[q][q] = sn * sn * app + 2.0 * c * sn * apq + c * c * aqq;
+                    a[p][q] = a[q][p] = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {              // V <- V J
+                        const double vkp = v[k][p], vkq = v[k][q];
+                        v[k][p] = c * vkp - sn * vkq; v[k][q] = sn * vkp + c * vkq;
+                    }
                 }
             }
     }
     double lmax = 0.0;
-    for (int i = 0; i < 6; ++i) { if (!isfinite(a[i][i])) return false; if (a[i][i] > lmax) lmax = a[i][i]; }
-    if (!(lmax > 0.0)) return false;
-    for (int i = 0; i < 6; ++i) if (a[i][i] < -1e-10 * lmax) return false;
+    bool finite = true;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { finite = finite && isfinite(a[i][i]); if (a[i][i] > lmax) lmax = a[i][i]; }
+    if (!finite || !(lmax > 0.0)) return false;
+    double inv[6];
+    bool negative = false;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        negative = negative || a[i][i] < -1e-10 * lmax;
+        inv[i] = a[i][i] > 1e-10 * lmax ? 1.0 / a[i][i] : 0.0;
+    }
+    if (negative) return false;
+#pragma unroll
     for (int r = 0; r < 6; ++r)
+#pragma unroll
         for (int c = 0; c < 6; ++c) {
             double sum = 0.0;
-            for (int i = 0; i < 6; ++i) if (a[i][i] > 1e-10 * lmax) sum += v[r][i] * v[c][i] / a[i][i];
+#pragma unroll
+            for (int i = 0; i < 6; ++i) sum += v[r][i] * v[c][i] * inv[i];
             out[6 * r + c] = sum;
         }
     return true;
@@ -595,7 +658,8 @@ __device__ __forceinline__ void sweep_step(double (&A)[kRT][kRT], bool has_tile,
 }
 
 template <bool WALL>
-__global__ void __maxnreg__(200)        // 160 threads x 200 registers: two CTAs per SM, no spills
+// Two CTAs per SM need <= 168 registers: each SM sub-partition holds 16,384 and gets three of the ten warps.
+__global__ void __launch_bounds__(kRegMaxThreads, 2)
 precond_build_reg_kernel(const double* __restrict__ pos, const double* __restrict__ q,
                          const int64_t* __restrict__ offsets, const int64_t* __restrict__ mat_off,
                          int* __restrict__ info, double* __restrict__ factors, double* __restrict__ Yg,
@@ -736,19 +800,32 @@ __global__ void precond_finish_kernel(const int* __restrict__ info, int64_t n_bo
 }
 
 // ------------------------------------------------------------------ preconditioner apply
-// One warp per body: [lambda; U] = P_p^-1 [x; y] (Eq. (19)):
+// [lambda; U] = P_p^-1 [x; y] (Eq. (19)):
 //   r = Y^T x (= K^T M^-1 x),  U = -N~ (y + r),  t = M^-1 x,  lambda = t + Y U.
-// One warp per body.  t = (M^(pp))^-1 x is a dense symmetric matrix-vector product: lane l owns
-// rows l, l+32, ... in chunks of 128 rows and walks the columns j, reading the contiguous row j of
-// the stored inverse (= its column j) -- coalesced, every load independent of the arithmetic, so the
-// kernel streams the inverses at memory speed instead of waiting on 2m dependent substitution steps.
-__global__ void precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
-                                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies,
-                                     int64_t vec_stride /* between right-hand sides (blockIdx.y) */,
-                                     float* __restrict__ lam32 /* optional float copy of lambda, [rhs][3 n_blobs] */)
+// t = (M^(pp))^-1 x is a dense symmetric matrix-vector product: lane l owns rows l, l+32, ... in chunks of 128
+// rows and walks the columns j, reading the contiguous row j of the stored inverse (= its column j) --
+// coalesced, every load independent of the arithmetic, so the kernel streams the inverses at memory speed
+// instead of waiting on 2m dependent substitution steps.
+// WPB warps per body (CTA of 128 threads = 4 / WPB bodies): with WPB = 4 each warp takes a quarter of the
+// columns and the four partial sums are added through shared memory in a fixed order -- four times as many
+// loads in flight when there are too few bodies to fill the GPU with one warp each.
+// With `vnorm` set the input is first scaled, v = scal[rhs][1] * in (the Arnoldi normalisation v_{j+1} = w / h_{j+1,j},
+// or r / beta at the start of a cycle), v is stored to vnorm as the new Krylov vector and the kernel applies P^-1
+// to it: the normalisation costs no launch of its own.
+template <int WPB>
+__global__ void __launch_bounds__(128)
+precond_apply_kernel(const void* __restrict__ precond, const double* __restrict__ in,
+                     double* __restrict__ out, int64_t n_blobs, int64_t n_bodies,
+                     int64_t vec_stride /* between right-hand sides (blockIdx.y) */,
+                     float* __restrict__ lam32 /* optional float copy of lambda, [rhs][3 n_blobs] */,
+                     const double* __restrict__ scal, double* __restrict__ vnorm,
+                     const int* __restrict__ skip)
 {
-    const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    __shared__ double red[WPB > 1 ? WPB : 1][128];
+    if (skip != nullptr && *skip != 0) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t p = (int64_t)blockIdx.x * (4 / WPB) + warp / WPB;
+    const int part = warp % WPB;
     in += (int64_t)blockIdx.y * vec_stride; out += (int64_t)blockIdx.y * vec_stride;
     if (lam32) lam32 += (int64_t)blockIdx.y * 3 * n_blobs;
     const int64_t* hdr = static_cast<const int64_t*>(precond);
@@ -759,24 +836,30 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
             out[i] = __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
-    if (p >= n_bodies) return;
+    if (p >= n_bodies) return;                       // WPB > 1: the whole CTA (one body) returns together
     const PrecondView pv = view_of(const_cast<void*>(precond), n_bodies, n_blobs, hdr[3]);
     const int64_t b0 = pv.offsets[p];
     const int m = 3 * (int)(pv.offsets[p + 1] - b0);
     const double* __restrict__ S = pv.factors + pv.mat_off[p];
     const double* __restrict__ Y = pv.Y + b0 * 18;
     const double* __restrict__ x = in + 3 * b0;
-    const double* y = in + 3 * n_blobs + 6 * p;
+    const double* __restrict__ y = in + 3 * n_blobs + 6 * p;
+    const double sc = vnorm ? scal[(int64_t)blockIdx.y * kScal + 1] : 1.0;     // every read of x, y below is sc * (.)
+    if (vnorm && part == 0) {
+        double* v = vnorm + (int64_t)blockIdx.y * vec_stride;
+        for (int i = lane; i < m; i += 32) v[3 * b0 + i] = sc * x[i];
+        if (lane < 6) v[3 * n_blobs + 6 * p + lane] = sc * y[lane];
+    }
     double* t = out + 3 * b0;
 
-    double r[6] = {0, 0, 0, 0, 0, 0};
+    double r[6] = {0, 0, 0, 0, 0, 0};                // every warp of the body forms r and U itself (m x 6 loads)
     for (int i = lane; i < m; i += 32) {
-        const double xi = x[i];
+        const double xi = sc * x[i];
 #pragma unroll
         for (int c = 0; c < 6; ++c) r[c] += Y[(size_t)i * 6 + c] * xi;
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) r[c] = warp_sum(r[c]) + y[c];
+    for (int c = 0; c < 6; ++c) r[c] = warp_sum(r[c]) + sc * y[c];
     double U[6];
 #pragma unroll
     for (int a = 0; a < 6; ++a) {
@@ -785,41 +868,58 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
         for (int c = 0; c < 6; ++c) s += pv.Nt[(size_t)p * 36 + 6 * a + c] * r[c];
         U[a] = -s;
     }
+    const int j_lo = (int)((int64_t)m * part / WPB), j_hi = (int)((int64_t)m * (part + 1) / WPB);
     for (int i0 = 0; i0 < m; i0 += 128) {
         const int i_a = i0 + lane, i_b = i_a + 32, i_c = i_a + 64, i_d = i_a + 96;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
         if (i0 + 128 <= m) {
 #pragma unroll 4
-            for (int j = 0; j < m; ++j) {
+            for (int j = j_lo; j < j_hi; ++j) {
                 const double* row = S + (size_t)j * m;
-                const double xj = x[j];
+                const double xj = sc * x[j];
                 a0 += row[i_a] * xj; a1 += row[i_b] * xj; a2 += row[i_c] * xj; a3 += row[i_d] * xj;
             }
         } else {
 #pragma unroll 4
-            for (int j = 0; j < m; ++j) {
+            for (int j = j_lo; j < j_hi; ++j) {
                 const double* row = S + (size_t)j * m;
-                const double xj = x[j];
+                const double xj = sc * x[j];
                 if (i_a < m) a0 += row[i_a] * xj;
                 if (i_b < m) a1 += row[i_b] * xj;
                 if (i_c < m) a2 += row[i_c] * xj;
                 if (i_d < m) a3 += row[i_d] * xj;
             }
         }
-        const int idx[4] = {i_a, i_b, i_c, i_d};
-        const double acc[4] = {a0, a1, a2, a3};
+        if (WPB == 1) {
+            const int idx[4] = {i_a, i_b, i_c, i_d};
+            const double acc[4] = {a0, a1, a2, a3};
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (idx[k] < m) {
-                double s = acc[k];
+            for (int k = 0; k < 4; ++k) {
+                if (idx[k] < m) {
+                    double s = acc[k];
 #pragma unroll
-                for (int c = 0; c < 6; ++c) s += Y[(size_t)idx[k] * 6 + c] * U[c];
-                t[idx[k]] = s;
-                if (lam32) lam32[3 * b0 + idx[k]] = (float)s;
+                    for (int c = 0; c < 6; ++c) s += Y[(size_t)idx[k] * 6 + c] * U[c];
+                    t[idx[k]] = s;
+                    if (lam32) lam32[3 * b0 + idx[k]] = (float)s;
+                }
             }
+        } else {
+            red[part][lane] = a0; red[part][lane + 32] = a1; red[part][lane + 64] = a2; red[part][lane + 96] = a3;
+            __syncthreads();
+            const int i = i0 + (int)threadIdx.x;          // one row per thread, the warps' shares in a fixed order
+            if (i < m) {
+                double s = red[0][threadIdx.x];
+#pragma unroll
+                for (int w = 1; w < WPB; ++w) s += red[w][threadIdx.x];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) s += Y[(size_t)i * 6 + c] * U[c];
+                t[i] = s;
+                if (lam32) lam32[3 * b0 + i] = (float)s;
+            }
+            __syncthreads();
         }
     }
-    if (lane < 6) {
+    if (part == 0 && lane < 6) {
         double v = U[0];
 #pragma unroll
         for (int c = 1; c < 6; ++c) if (lane == c) v = U[c];
@@ -834,9 +934,13 @@ __global__ void precond_apply_kernel(const void* __restrict__ precond, const dou
 // r is at V + (v * nrhs + r) * ldv.  A fixed grid of kVecBlocks CTAs cuts [0, n) into equal
 // contiguous chunks; every reduction is two-stage (per-CTA partials, then a fixed-order sum), so the
 // solve is bit-reproducible whenever the matvec is.
-constexpr int kVecBlocks = 296;       // 2 CTAs per SM
-constexpr int kVecThreads = 256;
-constexpr int kScal = 8;              // doubles of scalar state per right-hand side
+//
+// One Arnoldi step ("GMRES"; reading A16) is seven launches:
+//   precond_apply (v_j = w / h_{j,j-1} fused in), prepack, all-pairs, saddle_tail (finalise fused in),
+//   dots, update (second pass's dots fused in), update (norm, Hessenberg/Givens and the convergence test
+//   fused in: done by whichever CTA finishes last, in a fixed order).
+// The convergence test sets ctl[0]; every kernel of a later step returns at once when it is set, so the host
+// may enqueue step j+1 before it has read the outcome of step j.
 
 __device__ __forceinline__ void chunk_of(int64_t n, int64_t& lo, int64_t& hi)
 {
@@ -846,16 +950,13 @@ __device__ __forceinline__ void chunk_of(int64_t n, int64_t& lo, int64_t& hi)
     if (lo > n) lo = n;
 }
 
-// partial[(r * pvec + v) * gridDim.x + blk] = sum over the CTA's chunk of V[v][r][i] * w[r][i].
-// Warp w of the CTA takes v = w, w + 8, ...; no CTA barrier.
-__global__ void __launch_bounds__(kVecThreads)
-dots_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, const double* __restrict__ w, int64_t n,
-            double* __restrict__ partial, int pvec)
+// partial[(r * pvec + v) * gridDim.x + blk] = sum over the CTA's chunk of V[v][r][i] * w[r][i], warp w of the CTA
+// takes v = w, w + 8, ...
+__device__ __forceinline__ void chunk_dots(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec,
+                                           const double* __restrict__ wr, int64_t lo, int64_t hi,
+                                           double* __restrict__ partial, int pvec)
 {
-    const int r = blockIdx.y;
-    int64_t lo, hi; chunk_of(n, lo, hi);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const double* wr = w + (int64_t)r * ldv;
+    const int r = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int v = warp; v < nvec; v += kVecThreads / 32) {
         const double* a = V + ((int64_t)v * nrhs + r) * ldv;
         double s = 0.0;
@@ -865,15 +966,97 @@ dots_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, const
     }
 }
 
+__global__ void __launch_bounds__(kVecThreads)
+dots_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, const double* __restrict__ w, int64_t n,
+            double* __restrict__ partial, int pvec, const int* __restrict__ skip)
+{
+    if (skip != nullptr && *skip != 0) return;
+    int64_t lo, hi; chunk_of(n, lo, hi);
+    chunk_dots(V, ldv, nrhs, nvec, w + (int64_t)blockIdx.y * ldv, lo, hi, partial, pvec);
+}
+
+// Small state of one GMRES cycle, all on the device; every array has one slice per right-hand side
+// (slice r of an array with `len` entries per right-hand side starts at r * len).
+struct GmresState {
+    double* R;        // [(restart+1) * restart] column-major rotated Hessenberg (upper triangular after rotation)
+    double* cs;       // [restart]
+    double* sn;       // [restart]
+    double* g;        // [restart+1] rotated right-hand side
+    double* hcol;     // [restart+1] current Hessenberg column (sum of the two Gram-Schmidt passes)
+    double* yv;       // [restart]   solution of R y = g
+    double* scal;     // [kScal] [0] beta or h_{j+1,j}; [1] its reciprocal; [2] |g_{j+1}|; [3] ||b||; [4] beta of this cycle
+    int* ctl;         // [0] Arnoldi steps done when this cycle was told to stop (0: running); [1] converged;
+                      // [2] ticket counter of the last-CTA election; [3] iterations done by the solve
+    unsigned char* snap;   // [2][kSnapBytes] what the host reads after step j, in slot j & 1 (the live state may already
+                           // belong to step j+1, which is enqueued before step j is read): int stop, converged,
+                           // iterations, pad; then |g_{j+1}| of every right-hand side
+    int restart;
+};
+
+// What the CTA that finishes an Arnoldi step last needs for the convergence test.
+struct StepEnd {
+    int enabled;              // 0: first Gram-Schmidt pass (no step end)
+    int j;                    // step index inside the cycle
+    int max_iter;
+    int mixed;                // the estimates are those of the fp32 operator: end the cycle, do not declare convergence
+    double tol;
+    double inner_reduction;   // mixed: a cycle may reduce its start residual by this factor
+    double inner_tol_factor;  // mixed: ... or reach this fraction of tol
+};
+
+// Column j of the Hessenberg matrix of right-hand side r: hcol[0..j] from Gram-Schmidt, h_{j+1,j} = hn;
+// earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").  One warp: the
+// lanes first stage the column and the rotations in shared memory (`stage`, 3 (restart + 2) doubles), then lane 0
+// walks the chain of rotations there instead of through dependent global loads.
+__device__ void hessenberg_update(const GmresState& st, int r, int j, double hn, double* stage)
+{
+    const int m = st.restart, ldr = m + 1, lane = threadIdx.x & 31;
+    double* scal = st.scal + (int64_t)r * kScal;
+    double* cs = st.cs + (int64_t)r * m; double* sn = st.sn + (int64_t)r * m;
+    double* g = st.g + (int64_t)r * ldr; const double* hcol = st.hcol + (int64_t)r * ldr;
+    double* col = stage; double* scs = stage + (m + 2); double* ssn = stage + 2 * (m + 2);
+    for (int i = lane; i <= j; i += 32) col[i] = __ldcg(hcol + i);   // written by another CTA of this launch
+    for (int i = lane; i < j; i += 32) { scs[i] = cs[i]; ssn[i] = sn[i]; }
+    __syncwarp();
+    if (lane == 0) {
+        scal[0] = hn;
+        scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
+        col[j + 1] = hn;
+        for (int i = 0; i < j; ++i) {
+            const double t = scs[i] * col[i] + ssn[i] * col[i + 1];
+            col[i + 1] = -ssn[i] * col[i] + scs[i] * col[i + 1];
+            col[i] = t;
+        }
+        const double d = hypot(col[j], col[j + 1]);
+        const double c = d > 0.0 ? col[j] / d : 1.0, sgn = d > 0.0 ? col[j + 1] / d : 0.0;
+        cs[j] = c; sn[j] = sgn;
+        col[j] = d; col[j + 1] = 0.0;
+        const double gj = g[j];
+        g[j + 1] = -sgn * gj;
+        g[j] = c * gj;
+        scal[2] = fabs(sgn * gj);
+    }
+    __syncwarp();
+    double* out = st.R + (int64_t)r * ldr * m + (size_t)j * ldr;
+    for (int i = lane; i <= j + 1; i += 32) out[i] = col[i];
+}
+
 // h[v] = sum_blk partial[r][v][blk] (fixed order);  w -= sum_v h[v] V[v];  norm_partial[r][blk] = |w chunk|^2;
 // CTA 0 also does hcol[r][v] = (accumulate ? hcol[r][v] : 0) + h[v].
+// First Gram-Schmidt pass (dots_out set): the CTA also leaves the second pass's dot products of its chunk.
+// Second pass (end.enabled): the CTA that finishes last adds the norm partials of every right-hand side in a
+// fixed order, h_{j+1,j} = sqrt(sum), updates the Hessenberg problems and takes the convergence decision.
 __global__ void __launch_bounds__(kVecThreads)
 update_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, double* __restrict__ w, int64_t n,
               const double* __restrict__ partial, int pvec, double* __restrict__ hcol, int accumulate,
-              double* __restrict__ norm_partial)
+              double* __restrict__ norm_partial, double* __restrict__ dots_out, GmresState st, StepEnd end,
+              const int* __restrict__ skip)
 {
     __shared__ double h[RPY_RIGID_MAX_RESTART + 1];
     __shared__ double red[kVecThreads / 32];
+    __shared__ double stage[RPY_RIGID_MAX_BATCH][3 * (RPY_RIGID_MAX_RESTART + 2)];
+    __shared__ int s_last;
+    if (skip != nullptr && *skip != 0) return;
     const int r = blockIdx.y;
     for (int v = threadIdx.x >> 5; v < nvec; v += kVecThreads / 32) {      // one warp per dot product
         double s = 0.0;
@@ -902,76 +1085,54 @@ update_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, dou
         for (int k = 0; k < kVecThreads / 32; ++k) s += red[k];
         norm_partial[(int64_t)r * gridDim.x + blockIdx.x] = s;
     }
-}
+    if (dots_out) chunk_dots(V, ldv, nrhs, nvec, wr, lo, hi, dots_out, pvec);    // after the barrier: the chunk of w is final
+    if (!end.enabled) return;
 
-// Small state of one GMRES cycle, all on the device; every array has one slice per right-hand side
-// (slice r of an array with `len` entries per right-hand side starts at r * len).
-struct GmresState {
-    double* R;        // [(restart+1) * restart] column-major rotated Hessenberg (upper triangular after rotation)
-    double* cs;       // [restart]
-    double* sn;       // [restart]
-    double* g;        // [restart+1] rotated right-hand side
-    double* hcol;     // [restart+1] current Hessenberg column (sum of the two Gram-Schmidt passes)
-    double* yv;       // [restart]   solution of R y = g
-    double* scal;     // [kScal] [0] beta or h_{j+1,j}; [1] its reciprocal; [2] |g_{j+1}|; [3] ||b||
-    int restart;
-};
-
-// Column j of the Hessenberg matrix of right-hand side r: hcol[0..j] from Gram-Schmidt, h_{j+1,j} = hn;
-// earlier Givens rotations, the new rotation, g update (Saad & Schultz; "GMRES").  One thread.
-__device__ void hessenberg_update(const GmresState& st, int r, int j, double hn)
-{
-    const int m = st.restart, ldr = m + 1;
-    double* scal = st.scal + (int64_t)r * kScal;
-    double* cs = st.cs + (int64_t)r * m; double* sn = st.sn + (int64_t)r * m;
-    double* g = st.g + (int64_t)r * ldr; const double* hcol = st.hcol + (int64_t)r * ldr;
-    scal[0] = hn;
-    scal[1] = hn > 0.0 ? 1.0 / hn : 0.0;
-    double* col = st.R + (int64_t)r * ldr * m + (size_t)j * ldr;
-    for (int i = 0; i <= j; ++i) col[i] = hcol[i];
-    col[j + 1] = hn;
-    for (int i = 0; i < j; ++i) {
-        const double t = cs[i] * col[i] + sn[i] * col[i + 1];
-        col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
-        col[i] = t;
-    }
-    const double d = hypot(col[j], col[j + 1]);
-    const double c = d > 0.0 ? col[j] / d : 1.0, sgn = d > 0.0 ? col[j + 1] / d : 0.0;
-    cs[j] = c; sn[j] = sgn;
-    col[j] = d; col[j + 1] = 0.0;
-    g[j + 1] = -sgn * g[j];
-    g[j] = c * g[j];
-    scal[2] = fabs(g[j + 1]);
-}
-
-// End of Arnoldi step j in ONE launch: every CTA sums the norm partials of its right-hand side
-// (blockIdx.y) in the same fixed order, h_{j+1,j} = sqrt(sum), and writes its chunk of
-// v_{j+1} = w / h_{j+1,j}; CTA 0 of each right-hand side also updates the Hessenberg problem.
-__global__ void __launch_bounds__(kVecThreads)
-normalise_kernel(GmresState st, int j, const double* __restrict__ norm_partial, const double* __restrict__ w,
-                 int64_t ldv, double* __restrict__ vnext, int64_t n)
-{
-    __shared__ double s_inv;
-    const int r = blockIdx.y, nblk = gridDim.x;
-    if (threadIdx.x < 32) {
-        double s = 0.0;                              // one warp: fixed-order strided sums, then shuffles
-        for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
+    // ---- end of the Arnoldi step: the last CTA to get here closes it
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&st.ctl[2], 1) == (int)(gridDim.x * gridDim.y) - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp < nrhs) {                                   // nrhs <= RPY_RIGID_MAX_BATCH = warps of the CTA
+        double s = 0.0;                                  // fixed-order strided sums, then shuffles
+        for (int b = lane; b < (int)gridDim.x; b += 32) s += __ldcg(norm_partial + (int64_t)warp * gridDim.x + b);
         s = warp_sum(s);
-        if (threadIdx.x == 0) {
-            const double hn = sqrt(s);
-            s_inv = hn > 0.0 ? 1.0 / hn : 0.0;
-            if (blockIdx.x == 0) hessenberg_update(st, r, j, hn);
-        }
+        hessenberg_update(st, warp, end.j, sqrt(s), stage[warp]);
     }
     __syncthreads();
-    const double inv = s_inv;
-    int64_t lo, hi; chunk_of(n, lo, hi);
-    const double* wr = w + (int64_t)r * ldv; double* o = vnext + (int64_t)r * ldv;
-    for (int64_t i = lo + threadIdx.x; i < hi; i += kVecThreads) o[i] = inv * wr[i];
+    if (threadIdx.x == 0) {
+        bool all_conv = true, inner_all = true;
+        for (int q = 0; q < nrhs; ++q) {
+            const double* sc = st.scal + (int64_t)q * kScal;
+            const double res = sc[2], bn = sc[3];
+            const double rel = bn > 0.0 ? res / bn : 0.0;
+            if (rel > end.tol) all_conv = false;
+            if (rel > end.inner_tol_factor * end.tol && res > end.inner_reduction * sc[4]) inner_all = false;
+        }
+        const int n_iter = st.ctl[3] + 1;
+        st.ctl[3] = n_iter;
+        st.ctl[2] = 0;
+        if (end.mixed) {
+            // estimates of the fp32 operator: end the cycle once every right-hand side has gained
+            // inner_reduction (or is safely below tol) and let the fp64 residual of the restart decide
+            if (inner_all || n_iter >= end.max_iter) st.ctl[0] = end.j + 1;
+        } else if (all_conv || n_iter >= end.max_iter) {
+            st.ctl[0] = end.j + 1;
+            st.ctl[1] = all_conv ? 1 : 0;
+        }
+        int* si = reinterpret_cast<int*>(st.snap + (size_t)(end.j & 1) * kSnapBytes);
+        double* sr = reinterpret_cast<double*>(si + 4);
+        si[0] = st.ctl[0]; si[1] = st.ctl[1]; si[2] = n_iter; si[3] = 0;
+        for (int q = 0; q < nrhs; ++q) sr[q] = st.scal[(int64_t)q * kScal + 2];
+    }
 }
 
-// beta = sqrt(sum partial) at the start of a cycle: g = (beta, 0, ...), scal[0..1] = beta, 1/beta;
-// with set_bnorm, scal[3] = beta (the first cycle starts from x0 = 0, so r0 = b).
+// beta = sqrt(sum partial) at the start of a cycle: g = (beta, 0, ...), scal[0..1] = beta, 1/beta, scal[4] = beta;
+// with set_bnorm, scal[3] = beta (the first cycle starts from x0 = 0, so r0 = b) and the iteration count is
+// cleared.  The cycle's stop flag is cleared.
 __global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int set_bnorm)
 {
     const int r = blockIdx.x, ldr = st.restart + 1;
@@ -982,9 +1143,13 @@ __global__ void cycle_start_kernel(GmresState st, const double* __restrict__ nor
     double* scal = st.scal + (int64_t)r * kScal;
     double* g = st.g + (int64_t)r * ldr;
     const double beta = sqrt(s);
-    scal[0] = beta; scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; scal[2] = beta;
+    scal[0] = beta; scal[1] = beta > 0.0 ? 1.0 / beta : 0.0; scal[2] = beta; scal[4] = beta;
     if (set_bnorm) scal[3] = beta;
     for (int i = 0; i < ldr; ++i) g[i] = i == 0 ? beta : 0.0;
+    if (r == 0) {
+        st.ctl[0] = 0; st.ctl[1] = 0; st.ctl[2] = 0;
+        if (set_bnorm) st.ctl[3] = 0;
+    }
 }
 
 // R y = g for the first k columns (back substitution); a zero pivot (a right-hand side that was
@@ -1001,16 +1166,6 @@ __global__ void solve_y_kernel(GmresState st, int k)
         const double piv = R[(size_t)i * ldr + i];
         yv[i] = piv != 0.0 ? s / piv : 0.0;
     }
-}
-
-// out[r][i] = scal[r][which] * in[r][i]
-__global__ void scale_kernel(const double* __restrict__ in, int64_t in_stride, const double* __restrict__ scal, int which,
-                             double* __restrict__ out, int64_t out_stride, int64_t n)
-{
-    const int r = blockIdx.y;
-    const double s = scal[(int64_t)r * kScal + which];
-    const double* a = in + (int64_t)r * in_stride; double* o = out + (int64_t)r * out_stride;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = s * a[i];
 }
 
 // out[r][i] = sum_{v<k} y[r][v] V[v][r][i]
@@ -1053,8 +1208,10 @@ norm_partial_kernel(const double* __restrict__ w, int64_t ldv, int64_t n, double
     }
 }
 
-__global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride, float* __restrict__ out, int64_t out_stride, int64_t n)
+__global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride, float* __restrict__ out, int64_t out_stride, int64_t n,
+                                const int* __restrict__ skip = nullptr)
 {
+    if (skip != nullptr && *skip != 0) return;
     const double* a = in + (int64_t)blockIdx.y * in_stride; float* o = out + (int64_t)blockIdx.y * out_stride;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (float)a[i];
 }
@@ -1109,14 +1266,21 @@ rpy_status check_bodies(int64_t n_blobs, int64_t n_bodies)
 }
 
 constexpr rpy_prec kPrecMixed = static_cast<rpy_prec>(RPY_PREC_MIXED);
-constexpr double kInnerReduction = 1e-4;     // residual reduction asked of one fp32 cycle (mixed solve)
+// Mixed solve (reading A21): a cycle of fp32 products ends once its residual estimate has fallen by
+// kInnerReduction or is below kInnerTolFactor * tol; the fp64 residual of the restart then decides.  Measured
+// (B200, tol 1e-8): 1e-4 / 1.0 needs 45 (cfg 2) and 23 (cfg 3) iterations and two fp64 products; a deeper
+// first cycle with a safety margin on the second (1e-5 / 0.5) needs 47 and 25 iterations for the same two
+// fp64 products -- every restart discards the Krylov space, so the shallower split wins.
+constexpr double kInnerReduction = 1e-4;
+constexpr double kInnerTolFactor = 1.0;
 
 // Solver workspace, carved from one caller-owned buffer (nrhs lockstep right-hand sides).
 struct SolveWs {
     int64_t n; size_t vec_bytes; int nrhs;
     double *V, *w, *z, *x, *b;
     GmresState st;
-    double *partial, *norm_partial;
+    double *partial, *partial2, *norm_partial;
+    unsigned char* status;            // [64 bytes: ctl ints][kScal doubles per right-hand side]: one read-back
     float *pos32, *lam32, *vel32;
     void* mv; size_t mv_bytes;
     size_t total;
@@ -1124,7 +1288,8 @@ struct SolveWs {
 
 size_t mv_bytes_of(rpy_prec prec, int64_t n_blobs, int nrhs)
 {
-    if (prec != kPrecMixed) return rpy_matvec_workspace_bytes(prec, n_blobs, nrhs);
+    // every solve also forms fp64 residuals (the mixed solve per cycle, the fp32 solve once at the end)
+    if (prec == RPY_PREC_F64) return rpy_matvec_workspace_bytes(prec, n_blobs, nrhs);
     const size_t a = rpy_matvec_workspace_bytes(RPY_PREC_F64, n_blobs, nrhs), b = rpy_matvec_workspace_bytes(RPY_PREC_F32_ACC64, n_blobs, nrhs);
     return a > b ? a : b;
 }
@@ -1146,8 +1311,12 @@ SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, int
     W.st.R = (double*)take((size_t)(restart + 1) * restart * 8 * k);
     W.st.cs = (double*)take((size_t)restart * 8 * k); W.st.sn = (double*)take((size_t)restart * 8 * k);
     W.st.g = (double*)take((size_t)(restart + 1) * 8 * k); W.st.hcol = (double*)take((size_t)(restart + 1) * 8 * k);
-    W.st.yv = (double*)take((size_t)restart * 8 * k); W.st.scal = (double*)take((size_t)kScal * 8 * k);
+    W.st.yv = (double*)take((size_t)restart * 8 * k);
+    W.status = take(64 + (size_t)kScal * 8 * k);
+    W.st.ctl = (int*)W.status; W.st.scal = (double*)(p ? W.status + 64 : nullptr);
+    W.st.snap = take(2 * kSnapBytes);
     W.partial = (double*)take((size_t)kVecBlocks * (restart + 1) * 8 * k);
+    W.partial2 = (double*)take((size_t)kVecBlocks * (restart + 1) * 8 * k);
     W.norm_partial = (double*)take((size_t)kVecBlocks * 8 * k);
     if (prec != RPY_PREC_F64) {
         W.pos32 = (float*)take((size_t)n_blobs * 12); W.lam32 = (float*)take((size_t)n_blobs * 12 * k);
@@ -1162,31 +1331,64 @@ SolveWs carve(rpy_prec prec, int64_t n_blobs, int64_t n_bodies, int restart, int
 inline int64_t vec_stride(const SolveWs& W) { return (int64_t)(W.vec_bytes / 8); }
 inline dim3 vgrid(int nrhs) { return dim3(kVecBlocks, (unsigned)nrhs); }
 
+// How one rank's share of the product is completed (include/rpy_rigid.h, rpy_rigid_solve_ext).
+struct ShardCtx { int shard = 0, n_shards = 1; rpy_reduce_fn reduce = nullptr; void* ctx = nullptr; };
+
 // out[r] = [M lambda_r - K U_r ; -K^T lambda_r] for the nrhs solver vectors in[r] (stride `stride`):
 // Eq. (11)'s operator; ONE product call with n_rhs = nrhs.  pos32 must hold float(pos) for the fp32 product.
+// skip: device flag that turns the whole application into a no-op (see "Krylov vector operations").
 rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* pos, const double* q,
                   const int64_t* off, double a, double eta, const double* in, double* out, int64_t stride,
-                  int nrhs, const SolveWs& W, cudaStream_t st, bool lam32_ready = false)
+                  int nrhs, const SolveWs& W, cudaStream_t st, bool lam32_ready = false, const int* skip = nullptr,
+                  const ShardCtx& sh = ShardCtx{})
 {
     rpy_status s;
-    if (prec == RPY_PREC_F64) {
-        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, pos, in, stride, out, stride, a, eta, W.mv, W.mv_bytes, st);
-        if (s != RPY_OK) return s;
-    } else {
-        if (!lam32_ready) to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N);
-        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st);
-        if (s != RPY_OK) return s;
-    }
+    const bool f64 = prec == RPY_PREC_F64;
+    if (!f64 && !lam32_ready) to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N, skip);
+    const void* mpos = f64 ? (const void*)pos : (const void*)W.pos32;
+    const void* mforce = f64 ? (const void*)in : (const void*)W.lam32;
+    const int64_t fstride = f64 ? stride : 3 * N;
     const dim3 bg(warp_grid(nb, 128), (unsigned)nrhs);
-    saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, prec == RPY_PREC_F64 ? nullptr : W.vel32, out, N, nb, stride);
+    rpy::PartialSums ps{nullptr, 0, 0, 0.0};
+    if (sh.n_shards > 1) {
+        // this rank's share of the unordered pairs, as doubles, straight into out; the caller's hook adds the ranks
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, mpos, mforce, fstride, out, stride, a, eta, W.mv, W.mv_bytes, st,
+                                skip, nullptr, sh.shard, sh.n_shards, true);
+        if (s != RPY_OK) return s;
+        if (sh.reduce(sh.ctx, out, 3 * N, st) != 0) return RPY_ERR_ARG;
+        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+    } else if (nrhs == 1 || nrhs == 2 || nrhs == 4 || nrhs == 8) {
+        // one right-hand-side group: the product stops before its finalise step, the tail adds the slices
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, mpos, mforce, fstride, nullptr, 0, a, eta, W.mv, W.mv_bytes, st,
+                                skip, &ps);
+        if (s != RPY_OK) return s;
+        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+    } else if (f64) {
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, pos, in, stride, out, stride, a, eta, W.mv, W.mv_bytes, st, skip);
+        if (s != RPY_OK) return s;
+        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+    } else {
+        s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st, skip);
+        if (s != RPY_OK) return s;
+        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, W.vel32, out, N, nb, stride, ps, skip);
+    }
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
 
+// [lambda; U] = P^-1 in; with `vnorm` the input is first scaled by scal[rhs][1] and stored there (see the kernel).
 rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const double* in, double* out, int64_t stride,
-                         int nrhs, cudaStream_t st, float* lam32 = nullptr)
+                         int nrhs, cudaStream_t st, float* lam32 = nullptr, const double* scal = nullptr,
+                         double* vnorm = nullptr, const int* skip = nullptr)
 {
-    precond_apply_kernel<<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32);
+    // one warp per body streams the inverses at HBM speed once there are enough bodies; below that four warps
+    // per body (a CTA each) keep more loads in flight
+    if (nb >= 8192)
+        precond_apply_kernel<1><<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32,
+                                                                                        scal, vnorm, skip);
+    else
+        precond_apply_kernel<4><<<dim3((unsigned)nb, (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32,
+                                                                                  scal, vnorm, skip);
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -1289,6 +1491,9 @@ rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, 
     if (max_small > 0) {
         const int TA = (max_small + kRT - 1) / kRT + 1;
         const int threads = (TA * (TA + 1) / 2 + 31) / 32 * 32;
+        // 22 KB of panels per CTA: ask for a carve-out that lets the register-limited two CTAs per SM in
+        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_reg_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 50));
+        RPY_CUDA_TRY(cudaFuncSetAttribute(precond_build_reg_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 50));
         if (wall) precond_build_reg_kernel<true><<<(unsigned)n_bodies, threads, 0, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
                                                                                        v.factors, v.Y, v.Nt, 1.0 / a, scale);
         else      precond_build_reg_kernel<false><<<(unsigned)n_bodies, threads, 0, st>>>(d_pos, d_q, v.offsets, v.mat_off, v.info,
@@ -1406,38 +1611,45 @@ rpy_status rpy_rigid_saddle_apply(int wall, rpy_prec matvec_prec, int64_t n_blob
 
 namespace {
 
-// A second stream and an event that live for the duration of one solve: the residual norm travels to
-// the host on the side stream while the main stream already applies the preconditioner of the NEXT
-// iteration, so the host's read-back latency is covered by device work (the speculative application
-// is wasted only in the last iteration).
-struct SideStream {
-    cudaStream_t s2 = nullptr; cudaEvent_t ev = nullptr;
-    cudaError_t init()
-    {
-        cudaError_t e = cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking);
-        return e != cudaSuccess ? e : cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
-    }
-    ~SideStream() { if (ev) cudaEventDestroy(ev); if (s2) cudaStreamDestroy(s2); }
-};
-
 // nrhs GMRES processes in lockstep (one per right-hand side, sharing every kernel launch and ONE
 // product call with n_rhs = nrhs per iteration); nrhs = 1 is the plain solve.
+//
+// Host and device.  The device decides: the kernel that closes Arnoldi step j applies the stopping rule and sets
+// ctl[0]; the kernels of every later step return at once when it is set.  The host therefore enqueues step j+1
+// BEFORE it reads the outcome of step j (the 16 + 64 nrhs bytes of W.status), and reads it on the caller's side
+// stream, ordered after step j by the caller's event: the read-back and the host's launch work are covered by
+// device work, and a step enqueued in vain costs seven empty kernels.  Without a side stream the host reads on
+// the main stream and the device idles while the next step is being enqueued.
 rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, int nrhs,
                        const double* d_pos, const double* d_q, const int64_t* d_offsets,
                        const double* d_F, const double* d_slip, double a, double eta,
                        const void* d_precond, double tol, int restart, int max_iter,
                        double* d_lambda, double* d_U, double* h_history, int* h_n_iter, double* h_rel_resid,
-                       void* d_workspace, size_t workspace_bytes, cudaStream_t st)
+                       void* d_workspace, size_t workspace_bytes, cudaStream_t st, const rpy_rigid_solve_ext* ext)
 {
     const bool mixed = matvec_prec == kPrecMixed;
     const rpy_prec inner_prec = mixed ? RPY_PREC_F32_ACC64 : matvec_prec;     // the product inside Arnoldi
     const rpy_prec outer_prec = mixed ? RPY_PREC_F64 : matvec_prec;           // the product of a restart's residual
     SolveWs W = carve(matvec_prec, N, nb, restart, nrhs, d_workspace);
     if (workspace_bytes < W.total || ((uintptr_t)d_workspace % kAlign) != 0) return RPY_ERR_WORKSPACE;
+    ShardCtx sh;
+    cudaStream_t side = nullptr; cudaEvent_t side_ev = nullptr;
+    if (ext) {
+        if (ext->n_shards < 1 || ext->shard < 0 || ext->shard >= ext->n_shards) return RPY_ERR_ARG;
+        if (ext->n_shards > 1) {
+            if (!ext->reduce) return RPY_ERR_NULL;
+            if (nrhs != 1 || !rpy::matvec_shardable(N)) return RPY_ERR_ARG;
+            sh.shard = ext->shard; sh.n_shards = ext->n_shards; sh.reduce = ext->reduce; sh.ctx = ext->reduce_ctx;
+        }
+        if (ext->side_stream && ext->side_event) {
+            side = static_cast<cudaStream_t>(ext->side_stream); side_ev = static_cast<cudaEvent_t>(ext->side_event);
+        }
+    }
     const int64_t n = W.n, ldv = vec_stride(W);
     const int pvec = restart + 1;
     const dim3 vg = vgrid(nrhs);
     float* const lam32_in_cycle = inner_prec == RPY_PREC_F64 ? nullptr : W.lam32;   // P^-1 also writes float(lambda)
+    const int* const ctl = W.st.ctl;
 
     int64_t bad = -1;
     rpy_status s = first_bad(nb, N, d_precond, &bad, st);
@@ -1451,91 +1663,120 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
     RPY_CUDA_TRY(cudaMemsetAsync(W.x, 0, W.vec_bytes * (size_t)nrhs, st));
     norm_partial_kernel<<<vg, kVecThreads, 0, st>>>(W.b, ldv, n, W.norm_partial);
     cycle_start_kernel<<<nrhs, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, 1);
-    double hs[RPY_RIGID_MAX_BATCH * kScal];
-    double bnorm[RPY_RIGID_MAX_BATCH], beta_cycle[RPY_RIGID_MAX_BATCH], rel[RPY_RIGID_MAX_BATCH];
-    auto read_scal = [&]() -> cudaError_t {
-        cudaError_t e = cudaMemcpyAsync(hs, W.st.scal, sizeof(double) * kScal * nrhs, cudaMemcpyDeviceToHost, st);
+
+    // one read-back: the four control words and the scalar state of every right-hand side
+    const size_t status_bytes = 64 + sizeof(double) * kScal * (size_t)nrhs;
+    alignas(8) unsigned char hbuf[64 + sizeof(double) * kScal * RPY_RIGID_MAX_BATCH];
+    const double* hs = reinterpret_cast<const double*>(hbuf + 64);
+    auto read_now = [&]() -> cudaError_t {           // after everything enqueued so far
+        cudaError_t e = cudaMemcpyAsync(hbuf, W.status, status_bytes, cudaMemcpyDeviceToHost, st);
         return e != cudaSuccess ? e : cudaStreamSynchronize(st);
     };
-    SideStream side;
-    RPY_CUDA_TRY(side.init());
-    // the same read-back, but ordered only after what the main stream has done SO FAR: work enqueued on
-    // the main stream between `mark` and `read_marked` overlaps the copy and the host's wait
-    auto mark = [&]() -> cudaError_t { return cudaEventRecord(side.ev, st); };
-    auto read_marked = [&]() -> cudaError_t {
-        cudaError_t e = cudaStreamWaitEvent(side.s2, side.ev, 0);
+    // the snapshot the device left at the end of step j (slot j & 1): read after what had been enqueued when
+    // mark() was called; step j+1, enqueued in between, writes the other slot
+    alignas(8) unsigned char hsnap[kSnapBytes];
+    const int* snap_i = reinterpret_cast<const int*>(hsnap);
+    const double* snap_res = reinterpret_cast<const double*>(hsnap + 16);
+    const size_t snap_bytes = 16 + sizeof(double) * (size_t)nrhs;
+    auto mark = [&]() -> cudaError_t { return side ? cudaEventRecord(side_ev, st) : cudaSuccess; };
+    auto read_marked = [&](int j) -> cudaError_t {
+        const unsigned char* src = W.st.snap + (size_t)(j & 1) * kSnapBytes;
+        if (!side) {
+            cudaError_t e = cudaMemcpyAsync(hsnap, src, snap_bytes, cudaMemcpyDeviceToHost, st);
+            return e != cudaSuccess ? e : cudaStreamSynchronize(st);
+        }
+        cudaError_t e = cudaStreamWaitEvent(side, side_ev, 0);
         if (e != cudaSuccess) return e;
-        e = cudaMemcpyAsync(hs, W.st.scal, sizeof(double) * kScal * nrhs, cudaMemcpyDeviceToHost, side.s2);
-        return e != cudaSuccess ? e : cudaStreamSynchronize(side.s2);
+        e = cudaMemcpyAsync(hsnap, src, snap_bytes, cudaMemcpyDeviceToHost, side);
+        return e != cudaSuccess ? e : cudaStreamSynchronize(side);
     };
-    RPY_CUDA_TRY(read_scal());
+    RPY_CUDA_TRY(read_now());
+    double bnorm[RPY_RIGID_MAX_BATCH], rel[RPY_RIGID_MAX_BATCH];
     bool any = false;
     for (int r = 0; r < nrhs; ++r) {
-        bnorm[r] = hs[r * kScal + 3]; beta_cycle[r] = bnorm[r];
+        bnorm[r] = hs[r * kScal + 3];
         if (!isfinite(bnorm[r])) return RPY_ERR_ARG;
         rel[r] = bnorm[r] > 0.0 ? 1.0 : 0.0;
         any = any || bnorm[r] > 0.0;
         if (h_history) h_history[(size_t)r * (max_iter + 1)] = rel[r];
     }
+    auto all_le = [&](const double* v, double t) { for (int r = 0; r < nrhs; ++r) if (v[r] > t) return false; return true; };
+
+    StepEnd end;
+    end.enabled = 1; end.j = 0; end.max_iter = max_iter; end.mixed = mixed ? 1 : 0; end.tol = tol;
+    end.inner_reduction = kInnerReduction; end.inner_tol_factor = kInnerTolFactor;
+    StepEnd no_end = end; no_end.enabled = 0;
+
+    // Arnoldi step j of the current cycle; `src` is what v_j is a multiple of (the residual for j = 0, else w)
+    auto enqueue_step = [&](int j, const double* src) -> rpy_status {
+        double* vj = W.V + (int64_t)j * nrhs * ldv;
+        rpy_status e = precond_apply(N, nb, d_precond, src, W.z, ldv, nrhs, st, lam32_in_cycle, W.st.scal, vj, ctl);
+        if (e != RPY_OK) return e;
+        e = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st,
+                   lam32_in_cycle != nullptr, ctl, sh);
+        if (e != RPY_OK) return e;
+        // classical Gram-Schmidt, twice (as accurate as the modified form; three launches for the two passes)
+        StepEnd ej = end; ej.j = j;
+        dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, ctl);
+        update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 0, W.norm_partial,
+                                                 W.partial2, W.st, no_end, ctl);
+        update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial2, pvec, W.st.hcol, 1, W.norm_partial,
+                                                 nullptr, W.st, ej, ctl);
+        RPY_CUDA_TRY(cudaGetLastError());
+        return RPY_OK;
+    };
+
     int n_iter = 0;
     const double* rvec = W.b;
     bool done = !any;
-    auto all_le = [&](const double* v, double t) { for (int r = 0; r < nrhs; ++r) if (v[r] > t) return false; return true; };
     while (!done) {
-        scale_kernel<<<vg, 256, 0, st>>>(rvec, ldv, W.st.scal, 1, W.V, ldv, n);          // v_0 = r / beta
         int k = 0;
-        bool z_ready = false;                    // W.z already holds P^-1 v_j (applied speculatively)
-        for (int j = 0; j < restart; ++j) {
-            const double* vj = W.V + (int64_t)j * nrhs * ldv;
-            if (!z_ready && (s = precond_apply(N, nb, d_precond, vj, W.z, ldv, nrhs, st, lam32_in_cycle)) != RPY_OK) return s;
-            z_ready = false;
-            if ((s = saddle(wall, inner_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.z, W.w, ldv, nrhs, W, st, lam32_in_cycle != nullptr)) != RPY_OK) return s;
-            ++n_iter;
-            // classical Gram-Schmidt, twice (as accurate as the modified form; two launches per pass)
-            dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
-            update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 0, W.norm_partial);
-            dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec);
-            update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 1, W.norm_partial);
-            normalise_kernel<<<vg, kVecThreads, 0, st>>>(W.st, j, W.norm_partial, W.w, ldv, W.V + (int64_t)(j + 1) * nrhs * ldv, n);
+        int enq = n_iter;                                    // iterations enqueued so far (those of step j included)
+        if ((s = enqueue_step(0, rvec)) != RPY_OK) return s;
+        ++enq;
+        for (int j = 0;; ++j) {
             RPY_CUDA_TRY(mark());
-            if (j + 1 < restart && n_iter < max_iter) {          // speculative: P^-1 v_{j+1} for the next iteration
-                if ((s = precond_apply(N, nb, d_precond, W.V + (int64_t)(j + 1) * nrhs * ldv, W.z, ldv, nrhs, st, lam32_in_cycle)) != RPY_OK) return s;
-                z_ready = true;
+            const bool more = j + 1 < restart && enq < max_iter;
+            if (more) {                                      // one step ahead of the device's decision
+                if ((s = enqueue_step(j + 1, W.w)) != RPY_OK) return s;
+                ++enq;
             }
-            RPY_CUDA_TRY(read_marked());
-            bool inner_all = true;
+            RPY_CUDA_TRY(read_marked(j));
+            ++n_iter;
             for (int r = 0; r < nrhs; ++r) {
-                const double res = hs[r * kScal + 2];
-                rel[r] = bnorm[r] > 0.0 ? res / bnorm[r] : 0.0;
+                rel[r] = bnorm[r] > 0.0 ? snap_res[r] / bnorm[r] : 0.0;
                 if (h_history) h_history[(size_t)r * (max_iter + 1) + n_iter] = rel[r];
-                if (rel[r] > tol && res > kInnerReduction * beta_cycle[r]) inner_all = false;
             }
             k = j + 1;
-            if (mixed) {
-                // the estimates are residuals of the fp32 operator: end the cycle once every right-hand side has
-                // gained kInnerReduction (or reached tol) and let the fp64 residual below decide
-                if (inner_all || n_iter >= max_iter) break;
-            } else if (all_le(rel, tol) || n_iter >= max_iter) { done = true; break; }
+            if (snap_i[0] != 0) {                            // the device closed the cycle at this step
+                if (!mixed) done = true;                     // converged, or max_iter reached
+                break;
+            }
+            if (!more) break;                                // restart length reached
         }
         // x += P^-1 (V_k y),  R y = g
         solve_y_kernel<<<nrhs, 32, 0, st>>>(W.st, k);
         combine_kernel<<<vg, 256, 0, st>>>(W.V, ldv, nrhs, k, W.st.yv, restart, W.w, n);
         if ((s = precond_apply(N, nb, d_precond, W.w, W.z, ldv, nrhs, st)) != RPY_OK) return s;
         axpby_kernel<<<vg, 256, 0, st>>>(1.0, W.z, ldv, 1.0, W.x, ldv, n);
-        if (done) break;
-        // restart: r = b - A x  (mixed solve: with the fp64 product -- the true residual of Eq. (11))
-        if ((s = saddle(wall, outer_prec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, ldv, nrhs, W, st)) != RPY_OK) return s;
+        const bool want_true_residual = matvec_prec != RPY_PREC_F64;     // the estimates were those of the fp32 operator
+        if (done && !want_true_residual) break;
+        if (!done && !mixed && n_iter >= max_iter) { done = true; if (!want_true_residual) break; }
+        // r = b - A x: the start of the next cycle; with fp32 products inside the cycle it is formed with the fp64
+        // product -- the true residual of Eq. (11), which decides convergence (mixed) or is what is reported (fp32)
+        const rpy_prec rprec = want_true_residual ? RPY_PREC_F64 : outer_prec;
+        if ((s = saddle(wall, rprec, N, nb, d_pos, d_q, d_offsets, a, eta, W.x, W.w, ldv, nrhs, W, st, false, nullptr, sh)) != RPY_OK) return s;
         axpby_kernel<<<vg, 256, 0, st>>>(1.0, W.b, ldv, -1.0, W.w, ldv, n);
         norm_partial_kernel<<<vg, kVecThreads, 0, st>>>(W.w, ldv, n, W.norm_partial);
         cycle_start_kernel<<<nrhs, 32, 0, st>>>(W.st, W.norm_partial, kVecBlocks, 0);
         rvec = W.w;
-        if (mixed) {
-            RPY_CUDA_TRY(read_scal());
+        if (want_true_residual) {
+            RPY_CUDA_TRY(read_now());
             for (int r = 0; r < nrhs; ++r) {
-                beta_cycle[r] = hs[r * kScal + 0];
-                rel[r] = bnorm[r] > 0.0 ? beta_cycle[r] / bnorm[r] : 0.0;
+                rel[r] = bnorm[r] > 0.0 ? hs[r * kScal + 0] / bnorm[r] : 0.0;
                 if (h_history) h_history[(size_t)r * (max_iter + 1) + n_iter] = rel[r];   // replace the estimate by the true value
             }
+            if (done) break;                                 // fp32 solve: reported, not iterated on
             if (all_le(rel, tol) || n_iter >= max_iter) done = true;
         }
     }
@@ -1553,7 +1794,7 @@ rpy_status solve_checked(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_
                          const double* d_F, const double* d_slip, double a, double eta,
                          const void* d_precond, double tol, int restart, int max_iter,
                          double* d_lambda, double* d_U, double* h_history, int* h_n_iter, double* h_rel_resid,
-                         void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+                         void* d_workspace, size_t workspace_bytes, void* cuda_stream, const rpy_rigid_solve_ext* ext)
 {
     if (matvec_prec != RPY_PREC_F64 && matvec_prec != RPY_PREC_F32_ACC64 && matvec_prec != kPrecMixed) return RPY_ERR_ARG;
     if (check_bodies(n_blobs, n_bodies) != RPY_OK || n_bodies < 1 || n_rhs < 1 || n_rhs > RPY_RIGID_MAX_BATCH) return RPY_ERR_ARG;
@@ -1562,7 +1803,7 @@ rpy_status solve_checked(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_
     if (!d_pos || !d_q || !d_offsets || !d_F || !d_precond || !d_lambda || !d_U || !d_workspace) return RPY_ERR_NULL;
     return solve_batch(wall, matvec_prec, n_blobs, n_bodies, n_rhs, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
                        tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
-                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+                       workspace_bytes, static_cast<cudaStream_t>(cuda_stream), ext);
 }
 
 }  // namespace
@@ -1575,11 +1816,12 @@ rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_bl
                                     const void* d_precond, double tol, int restart, int max_iter,
                                     double* d_lambda, double* d_U,
                                     double* h_history, int* h_n_iter, double* h_rel_resid,
-                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                                    const rpy_rigid_solve_ext* ext)
 {
     return solve_checked(wall, matvec_prec, n_blobs, n_bodies, 1, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
                          tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
-                         workspace_bytes, cuda_stream);
+                         workspace_bytes, cuda_stream, ext);
 }
 
 rpy_status rpy_rigid_mobility_solve_batch(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies, int n_rhs,
@@ -1588,11 +1830,12 @@ rpy_status rpy_rigid_mobility_solve_batch(int wall, rpy_prec matvec_prec, int64_
                                           const void* d_precond, double tol, int restart, int max_iter,
                                           double* d_lambda, double* d_U,
                                           double* h_history, int* h_n_iter, double* h_rel_resid,
-                                          void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+                                          void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                                          const rpy_rigid_solve_ext* ext)
 {
     return solve_checked(wall, matvec_prec, n_blobs, n_bodies, n_rhs, d_pos, d_q, d_offsets, d_F, d_slip, a, eta, d_precond,
                          tol, restart, max_iter, d_lambda, d_U, h_history, h_n_iter, h_rel_resid, d_workspace,
-                         workspace_bytes, cuda_stream);
+                         workspace_bytes, cuda_stream, ext);
 }
 
 }  // extern "C"

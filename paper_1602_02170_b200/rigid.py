@@ -25,6 +25,18 @@ RPY_RIGID_MAX_BATCH = 8
 _vp, _i64, _int, _dbl, _sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
 _i64p, _dblp, _intp = ctypes.POINTER(_i64), ctypes.POINTER(_dbl), ctypes.POINTER(_int)
 
+# int reduce(void* ctx, double* d_buf, int64_t count, void* cuda_stream): sums d_buf over the ranks in place
+REDUCE_FN = ctypes.CFUNCTYPE(_int, _vp, _vp, _i64, _vp)
+
+
+class SolveExt(ctypes.Structure):
+    """rpy_rigid_solve_ext: the caller's side stream and event, and the multi-GPU share of the product."""
+    _fields_ = [("side_stream", _vp), ("side_event", _vp), ("shard", _int), ("n_shards", _int),
+                ("reduce", REDUCE_FN), ("reduce_ctx", _vp)]
+
+
+_extp = ctypes.POINTER(SolveExt)
+
 SIGNATURES = {
     "rpy_rigid_K_apply": (_int, [_i64, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp]),
     "rpy_rigid_KT_apply": (_int, [_i64, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp]),
@@ -36,10 +48,10 @@ SIGNATURES = {
     "rpy_rigid_precond_get": (_int, [_i64, _i64p, _vp, _i64, _vp, _vp, _vp]),
     "rpy_rigid_solve_workspace_bytes": (_sz, [_int, _i64, _i64, _int]),
     "rpy_rigid_mobility_solve": (_int, [_int, _int, _i64, _i64, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _dbl,
-                                        _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp]),
+                                        _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp, _extp]),
     "rpy_rigid_solve_batch_workspace_bytes": (_sz, [_int, _i64, _i64, _int, _int]),
     "rpy_rigid_mobility_solve_batch": (_int, [_int, _int, _i64, _i64, _int, _vp, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp, _dbl,
-                                              _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp]),
+                                              _int, _int, _vp, _vp, _dblp, _intp, _dblp, _vp, _sz, _vp, _extp]),
     "rpy_rigid_saddle_apply": (_int, [_int, _int, _i64, _i64, _vp, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _sz, _vp]),
 }
 
@@ -174,13 +186,18 @@ class Precond:
 
 
 def rpy_rigid_precond_build(b: Bodies, variant: str = "wall", a: float = 1.0, eta: float = 1.0,
-                            check: bool = True) -> Precond:
-    """Dense M^(pp), its inverse via Cholesky, Y, N~ for every body (Eqs. (17)-(19)); `variant` 'wall' or 'free'."""
+                            check: bool = True, buf: Optional[torch.Tensor] = None) -> Precond:
+    """Dense M^(pp), its explicit inverse, Y, N~ for every body (Eqs. (17)-(19)); `variant` 'wall' or 'free'.
+    `buf`: a CUDA uint8 tensor of at least rpy_rigid_precond_bytes(offsets) bytes to build into (a time-stepping
+    caller rebuilds the preconditioner every step); allocated when None."""
     lib = _lib()
     need = int(lib.rpy_rigid_precond_bytes(b.n_bodies, _hptr(b.h_offsets)))
     if need == 0:
         raise ValueError("invalid body offsets (or a body above RPY_RIGID_MAX_BODY_BLOBS)")
-    buf = torch.empty(need, dtype=torch.uint8, device=b.pos.device)
+    if buf is None:
+        buf = torch.empty(need, dtype=torch.uint8, device=b.pos.device)
+    elif buf.dtype != torch.uint8 or not buf.is_cuda or not buf.is_contiguous() or buf.numel() < need:
+        raise ValueError(f"buf must be a contiguous CUDA uint8 tensor of at least {need} bytes")
     with torch.cuda.device(b.pos.device):
         _check(lib.rpy_rigid_precond_build(1 if variant == "wall" else 0, b.n_blobs, b.n_bodies, b.pos.data_ptr(),
                                            b.q.data_ptr(), _hptr(b.h_offsets), float(a), float(eta),
@@ -247,11 +264,55 @@ def rpy_rigid_saddle_apply(b: Bodies, x: torch.Tensor, variant: str = "wall", a:
     return out
 
 
+_side = {}          # (device index, thread) -> (side stream, event): created once, handed to every solve
+
+
+def _solve_ext(device, shard: int = 0, n_shards: int = 1, reduce=None, side: bool = True):
+    """(SolveExt, keep-alive objects): the side stream and event the solve reads its status on, and -- for a
+    multi-GPU solve -- this rank's share and the hook that sums the partial products over the ranks."""
+    ext = SolveExt()
+    keep = []
+    if side:
+        import threading
+        idx = torch.device(device).index
+        idx = torch.cuda.current_device() if idx is None else idx
+        key = (idx, threading.get_ident())                   # concurrent solves must not share an event
+        if key not in _side:
+            with torch.cuda.device(idx):
+                st, ev = torch.cuda.Stream(), torch.cuda.Event()
+                ev.record(torch.cuda.current_stream())       # torch creates the cudaEvent_t lazily
+                _side[key] = (st, ev)
+        st, ev = _side[key]
+        ext.side_stream, ext.side_event = st.cuda_stream, ev.cuda_event
+    ext.shard, ext.n_shards = int(shard), int(n_shards)
+    if n_shards > 1:
+        if reduce is None:
+            raise ValueError("a sharded solve needs a reduce hook")
+
+        def hook(_ctx, ptr, count, _stream):
+            try:
+                reduce(int(ptr), int(count))
+                return 0
+            except Exception:      # pragma: no cover
+                import traceback
+                traceback.print_exc()
+                return 1
+        cb = REDUCE_FN(hook)
+        keep.append(cb)
+        ext.reduce = cb
+    return ext, keep
+
+
 def rpy_rigid_mobility_solve(b: Bodies, pc: Precond, F: torch.Tensor, slip: Optional[torch.Tensor] = None,
                              variant: str = "wall", a: float = 1.0, eta: float = 1.0, tol: float = 1e-8,
                              restart: int = 60, max_iter: int = 200, matvec_prec="f64",
-                             workspace: Optional[torch.Tensor] = None) -> dict:
-    """Solves Eq. (11) by preconditioned GMRES.  Returns {'lambda', 'U', 'history', 'n_iter', 'rel_resid'}."""
+                             workspace: Optional[torch.Tensor] = None, shard: int = 0, n_shards: int = 1,
+                             reduce=None, side_stream: bool = True) -> dict:
+    """Solves Eq. (11) by preconditioned GMRES.  Returns {'lambda', 'U', 'history', 'n_iter', 'rel_resid'}.
+
+    Multi-GPU: every rank calls with the same arguments and its own ``shard`` of ``n_shards``;
+    ``reduce(ptr, count)`` must sum ``count`` doubles at device address ``ptr`` over the ranks in place, in
+    stream order on the current stream (``sharding.solve_reduce_hook`` binds it to torch.distributed)."""
     _f64(F, (b.n_bodies, 6), "F")
     if slip is not None:
         _f64(slip, (b.n_blobs, 3), "slip")
@@ -266,12 +327,14 @@ def rpy_rigid_mobility_solve(b: Bodies, pc: Precond, F: torch.Tensor, slip: Opti
     hist = (_dbl * (max_iter + 1))()
     n_iter, rel = _int(0), _dbl(0.0)
     with torch.cuda.device(b.pos.device):
+        ext, keep = _solve_ext(b.pos.device, shard, n_shards, reduce, side_stream)
         _check(_lib().rpy_rigid_mobility_solve(
             1 if variant == "wall" else 0, prec, b.n_blobs, b.n_bodies, b.pos.data_ptr(), b.q.data_ptr(),
             b.offsets.data_ptr(), F.data_ptr(), slip.data_ptr() if slip is not None else None, float(a), float(eta),
             pc.buf.data_ptr(), float(tol), int(restart), int(max_iter), lam.data_ptr(), U.data_ptr(),
             hist, ctypes.byref(n_iter), ctypes.byref(rel), workspace.data_ptr(), int(workspace.numel()),
-            _stream(b.pos)))
+            _stream(b.pos), ctypes.byref(ext)))
+    del keep
     return {"lambda": lam, "U": U, "history": list(hist[:n_iter.value + 1]), "n_iter": n_iter.value,
             "rel_resid": rel.value}
 
@@ -305,11 +368,13 @@ def rpy_rigid_mobility_solve_batch(b: Bodies, pc: Precond, F: torch.Tensor, slip
     hist = (_dbl * (k * (max_iter + 1)))()
     n_iter, rel = _int(0), (_dbl * k)()
     with torch.cuda.device(b.pos.device):
+        ext, _keep = _solve_ext(b.pos.device)
         _check(_lib().rpy_rigid_mobility_solve_batch(
             1 if variant == "wall" else 0, prec, b.n_blobs, b.n_bodies, k, b.pos.data_ptr(), b.q.data_ptr(),
             b.offsets.data_ptr(), F.data_ptr(), slip.data_ptr() if slip is not None else None, float(a), float(eta),
             pc.buf.data_ptr(), float(tol), int(restart), int(max_iter), lam.data_ptr(), U.data_ptr(),
-            hist, ctypes.byref(n_iter), rel, workspace.data_ptr(), int(workspace.numel()), _stream(b.pos)))
+            hist, ctypes.byref(n_iter), rel, workspace.data_ptr(), int(workspace.numel()), _stream(b.pos),
+            ctypes.byref(ext)))
     it = n_iter.value
     return {"lambda": lam, "U": U, "n_iter": it, "rel_resid": list(rel),
             "history": [list(hist[r * (max_iter + 1): r * (max_iter + 1) + it + 1]) for r in range(k)]}

@@ -89,3 +89,33 @@ def reduce_velocities(partial: torch.Tensor, group=None) -> torch.Tensor:
         raise TypeError("reduce_velocities: the partial products of rpy_*_matvec_shard are float64")
     dist.all_reduce(partial, op=dist.ReduceOp.SUM, group=group)
     return partial
+
+
+class _DevicePointer:
+    """Lets torch wrap `count` float64 values at a raw device address (CUDA array interface, version 2)."""
+
+    def __init__(self, ptr: int, count: int):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": "<f8", "data": (ptr, False), "version": 2}
+
+
+def wrap_doubles(ptr: int, count: int, device=None) -> torch.Tensor:
+    """A float64 tensor VIEW of `count` doubles at address `ptr`: device memory when `device` is a CUDA device,
+    else host memory.  No copy; the caller keeps the memory alive."""
+    if device is not None and torch.device(device).type == "cuda":
+        return torch.as_tensor(_DevicePointer(ptr, count), device=device)
+    import ctypes
+    import numpy as np
+    buf = (ctypes.c_double * count).from_address(ptr)
+    return torch.from_numpy(np.frombuffer(buf, dtype=np.float64, count=count))
+
+
+def solve_reduce_hook(group=None, device=None):
+    """The `reduce(ptr, count)` hook of a multi-GPU ``rpy_rigid_mobility_solve(..., shard, n_shards, reduce)``:
+    one in-place all-reduce (sum) per product over the ranks' partial velocities, ordered on the current
+    stream like every torch.distributed collective.  Every rank runs the same replicated Krylov process on
+    the summed product, so all ranks take the same decisions and return the same solution."""
+    import torch.distributed as dist
+
+    def reduce(ptr: int, count: int):
+        dist.all_reduce(wrap_doubles(ptr, count, device), op=dist.ReduceOp.SUM, group=group)
+    return reduce

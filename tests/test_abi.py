@@ -237,11 +237,19 @@ def test_rigid_host_arithmetic_and_argument_checks():
     assert lib.rpy_rigid_precond_build(1, 10, 2, one, one, off, 1.0, 1.0, one, 16, None) == 4
     assert lib.rpy_rigid_precond_apply(10, 2, one, one, one, None) == 3            # in aliases out
     n_it, rr = ctypes.c_int(), ctypes.c_double()
-    args = lambda tol, restart, ws: (1, 0, 10, 2, one, one, one, one, None, 1.0, 1.0, one, tol, restart, 50, one, one,
-                                     None, ctypes.byref(n_it), ctypes.byref(rr), one, ws, None)
+    args = lambda tol, restart, ws, ext=None: (1, 0, 10, 2, one, one, one, one, None, 1.0, 1.0, one, tol, restart, 50, one, one,
+                                               None, ctypes.byref(n_it), ctypes.byref(rr), one, ws, None, ext)
     assert lib.rpy_rigid_mobility_solve(*args(-1.0, 10, 1 << 30)) == 2
     assert lib.rpy_rigid_mobility_solve(*args(1e-8, 500, 1 << 30)) == 2
     assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, 64)) == 4
+    # the optional extras: a share of the product needs a reduction hook, one right-hand side and the symmetric kernel
+    big = 1 << 30
+    ext = rigid.SolveExt(); ext.shard, ext.n_shards = 2, 2
+    assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, big, ctypes.byref(ext))) == 2      # shard >= n_shards
+    ext.shard = 0
+    assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, big, ctypes.byref(ext))) == 1      # no hook
+    ext.reduce = rigid.REDUCE_FN(lambda c, p, n, s: 0)
+    assert lib.rpy_rigid_mobility_solve(*args(1e-8, 10, big, ctypes.byref(ext))) == 2      # 10 blobs: no symmetric kernel
 
 
 def test_rigid_and_sharded_bindings_refuse_cpu_tensors():

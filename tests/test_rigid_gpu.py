@@ -499,3 +499,129 @@ def test_table1_iteration_counts_of_the_sphere_lattices():
             assert abs(r["n_iter"] - int(r_[col])) <= 2, (nblob, phi, r["n_iter"], r_[col])
         print(f"{nblob}-blob spheres: iterations {got}, paper {[int(r_[col]) for r_ in rows]}")
         assert got == sorted(got)                                   # denser lattices need more iterations
+
+
+@pytest.mark.parametrize("s,eta", [(1e-6, 1e-3), (1e3, 2.0)])
+def test_solve_does_not_depend_on_the_unit_of_length(s, eta):
+    """The same body in other units (lengths x s, viscosity eta): with the force kept and the torque x s the
+    velocity is u / (s eta) and the angular velocity omega / (s^2 eta).  The 6x6 K^T M^-1 K mixes eta L,
+    eta L^2 and eta L^3 blocks, so the cut-off of its pseudo-inverse must be taken in units of the blob
+    radius (reading A18): a micron-sized colloid in SI units (s = 1e-6) has rotational eigenvalues 1e-12 of
+    the translational ones.  Boomerangs (regular 6x6) and a straight rod (rank 5), one body per solve so that
+    the block-diagonal preconditioner is exact and the comparison is not limited by the GMRES tolerance
+    (whose residual norm mixes velocity and force units)."""
+    rng = np.random.default_rng(11)
+    w = workloads.config2(seed=6, n_bodies=2)
+    hb = workloads.bodies_of(w)
+    ax = np.array([np.cos(0.4), np.sin(0.4), 0.0])
+    rod = np.array([60.0, 60.0, 3.0]) + np.outer(2.0 * (np.arange(21) - 10), ax)
+    cases = [(w.pos[:15], hb.q[0], None), (w.pos[15:], hb.q[1], None), (rod, rod[10], ax)]
+    for pos, q, axis in cases:
+        F = rng.standard_normal((1, 6))
+        if axis is not None:
+            F[0, 3:] -= (F[0, 3:] @ axis) * axis           # consistent load: no torque about the rod's axis
+        off = np.array([0, pos.shape[0]])
+
+        def solve(scale, visc):
+            db = rigid.bodies(dev(pos * scale), dev(q[None, :] * scale), off)
+            pc = rigid.rpy_rigid_precond_build(db, "wall", a=scale, eta=visc)
+            Fs = F.copy(); Fs[:, 3:] *= scale
+            r = rigid.rpy_rigid_mobility_solve(db, pc, dev(Fs), None, "wall", a=scale, eta=visc, tol=1e-12)
+            assert r["n_iter"] <= 2, r
+            return r["U"].cpu().numpy()[0], rigid.rpy_rigid_precond_get(pc, 0)[1].cpu().numpy()
+
+        U1, N1 = solve(1.0, 1.0)
+        Us, Ns = solve(s, eta)
+        assert np.abs(U1[3:]).max() > 0.0 and np.isfinite(Us).all()
+        assert rel(Us[:3] * (s * eta), U1[:3]) < 1e-9
+        assert rel(Us[3:] * (s * s * eta), U1[3:]) < 1e-9
+        D = np.concatenate([np.full(3, s ** -0.5), np.full(3, s ** -1.5)]) / np.sqrt(eta)
+        assert rel(Ns, D[:, None] * N1 * D[None, :]) < 1e-9   # N~(s) = D N~(1) D, rank-deficient rod included
+        if axis is not None:
+            assert abs(Us[3:] @ axis) < 1e-9 * np.abs(Us[3:]).max()
+
+
+def test_a_preconditioner_of_other_bodies_is_refused():
+    """A buffer built for the same number of bodies but another number of blobs: the solve returns
+    RPY_ERR_ARG (header check on the host) and the bare application poisons its output with NaN instead of
+    silently leaving it untouched."""
+    pos, b, lam, db = boomerangs(4)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    pos2 = np.concatenate([pos, pos[-15:] + np.array([50.0, 0.0, 0.0]), pos[:1] + np.array([0.0, 80.0, 0.0])])
+    off2 = np.array([0, 15, 30, 60, 76])                   # 4 bodies again, 76 blobs instead of 60
+    db2 = rigid.bodies(dev(pos2), dev(np.concatenate([b.q[:3], pos2[60:61]])), off2)
+    wrong = rigid.Precond(pc.buf, db2, "wall")
+    with pytest.raises(RpyError) as ei:
+        rigid.rpy_rigid_mobility_solve(db2, wrong, dev(np.ones((4, 6))), None, "wall")
+    assert ei.value.status == 2
+    out = rigid.rpy_rigid_precond_apply(wrong, dev(np.ones(db2.n)))
+    assert bool(torch.isnan(out).all())
+    assert rigid.rpy_rigid_precond_info(pc) == -1          # reading the outcome does not write to the buffer
+    before = pc.buf.clone()
+    rigid.rpy_rigid_precond_info(pc)
+    assert torch.equal(before, pc.buf)
+
+
+@pytest.mark.parametrize("prec,n_shards", [("f64", 2), ("f64", 3), ("mixed", 2)])
+def test_sharded_krylov_loop_matches_the_single_gpu_solve(prec, n_shards):
+    """the Krylov loop with the product split over ranks.  The ranks are emulated on this one GPU
+    by host threads, one stream each, every one running the whole replicated solve with its own shard of the
+    product; the reduction hook is a host barrier plus a fixed-order sum of the ranks' partial products (what
+    one NCCL all-reduce does on a multi-GPU node: tests/test_sharding_gloo.py covers that hook).  No kernel
+    waits on another: only the host threads do."""
+    import threading
+    from paper_1602_02170_b200 import sharding
+    pos, b, lam, db = boomerangs(300, seed=2)                 # 4,500 blobs: the symmetric kernel, shardable
+    rng = np.random.default_rng(12)
+    F = rng.standard_normal((b.n_bodies, 6)); slip = 0.1 * rng.standard_normal(pos.shape)
+    tol = 1e-9
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    single = rigid.rpy_rigid_mobility_solve(db, pc, dev(F), dev(slip), "wall", tol=tol, matvec_prec=prec)
+    bufs, out, errors = [None] * n_shards, [None] * n_shards, []
+    barrier = threading.Barrier(n_shards, timeout=300)
+
+    def worker(rank):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                my = rigid.bodies(dev(pos), dev(b.q), b.offsets)
+                my_pc = rigid.rpy_rigid_precond_build(my, "wall")
+
+                def reduce(ptr, count):
+                    mine = sharding.wrap_doubles(ptr, count, "cuda")
+                    stream.synchronize()                      # my partial product is complete
+                    bufs[rank] = mine
+                    barrier.wait()
+                    total = torch.zeros_like(mine)
+                    for r in range(n_shards):                 # the same order on every rank
+                        total += bufs[r]
+                    stream.synchronize()
+                    barrier.wait()                            # everybody has read everybody's partial
+                    mine.copy_(total)
+
+                out[rank] = rigid.rpy_rigid_mobility_solve(my, my_pc, dev(F), dev(slip), "wall", tol=tol, matvec_prec=prec,
+                                                           shard=rank, n_shards=n_shards, reduce=reduce)
+                stream.synchronize()
+        except Exception as e:      # pragma: no cover
+            errors.append(e)
+            barrier.abort()
+
+    threads = [threading.Thread(target=worker, args=(r,)) for r in range(n_shards)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for r in range(n_shards):
+        assert out[r]["n_iter"] == single["n_iter"] and out[r]["rel_resid"] <= tol
+        assert torch.equal(out[r]["U"], out[0]["U"]) and torch.equal(out[r]["lambda"], out[0]["lambda"])
+    eU = rel(out[0]["U"].cpu().numpy(), single["U"].cpu().numpy())
+    eh = np.abs(np.array(out[0]["history"]) / np.array(single["history"]) - 1.0).max()
+    print(f"sharded solve {prec} G={n_shards}: {single['n_iter']} iterations, U rel diff {eU:.2e}, history rel diff {eh:.2e}")
+    # fp64: the same Krylov process up to the order of the fp64 sums; mixed: the estimates of the fp32 cycles
+    # differ at the level of the fp32 product's own error
+    assert eU < 1e-7 and eh < (1e-5 if prec == "f64" else 1e-3)
+    # without a hook, or with more than one right-hand side, a share of the product is refused
+    with pytest.raises((RpyError, ValueError)):
+        rigid.rpy_rigid_mobility_solve(db, pc, dev(F), None, "wall", shard=0, n_shards=2)

@@ -113,3 +113,39 @@ def test_two_rank_gloo_work_sharding_all_reduce(tmp_path):
     a, b = np.load(tmp_path / "red_0.npy"), np.load(tmp_path / "red_1.npy")
     assert np.array_equal(a, b)                       # every rank ends with the same u
     assert np.allclose(a, ref, rtol=1e-13, atol=1e-15)
+
+
+def _hook_worker(rank, world, port, n, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    os.environ["OMP_NUM_THREADS"] = "2"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        w = workloads.config1(seed=6, n=n, k=1)
+        reduce = sharding.solve_reduce_hook()              # what a sharded solve calls after each product
+        lo, cnt = sharding.shard_rows(n, rank, world)
+        outs = []
+        for it in range(3):                                # three "iterations": a new lambda each time
+            lam = np.roll(w.force, it, axis=1)
+            mine = np.zeros_like(lam); mine[:, lo:lo + cnt] = lam[:, lo:lo + cnt]
+            buf = np.ascontiguousarray(oracle.matvec(oracle.WALL, w.pos, mine, w.a, w.eta)).ravel()
+            reduce(buf.ctypes.data, buf.size)              # raw address + count, as the C ABI hands them over
+            outs.append(buf.copy())
+        np.save(os.path.join(out_dir, f"hook_{rank}.npy"), np.stack(outs))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_gloo_solve_reduce_hook(tmp_path):
+    """The reduction hook of the sharded Krylov loop (rpy_rigid_solve_ext.reduce): a raw address and a count in,
+    the sum over the ranks in place, the same on every rank; the oracle stands in for the per-rank CUDA product."""
+    import oracle
+    world, n = 2, 131
+    mp.spawn(_hook_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    w = workloads.config1(seed=6, n=n, k=1)
+    a, b = np.load(tmp_path / "hook_0.npy"), np.load(tmp_path / "hook_1.npy")
+    assert np.array_equal(a, b)
+    for it in range(3):
+        ref = oracle.matvec(oracle.WALL, w.pos, np.roll(w.force, it, axis=1), w.a, w.eta).ravel()
+        assert np.allclose(a[it], ref, rtol=1e-13, atol=1e-15)
