@@ -15,6 +15,20 @@
 #include <stdint.h>
 #include "rpy_math.cuh"
 
+#ifndef RPY_SYM_UNROLL_F32
+#define RPY_SYM_UNROLL_F32 4      // inner-loop unroll of the symmetric kernel (measured)
+#endif
+#ifndef RPY_SYM_UNROLL_F64
+#define RPY_SYM_UNROLL_F64 4
+#endif
+
+#ifndef RPY_SYM_UNROLL_F32
+#define RPY_SYM_UNROLL_F32 4
+#endif
+#ifndef RPY_SYM_UNROLL_F64
+#define RPY_SYM_UNROLL_F64 4
+#endif
+
 namespace rpy {
 
 template <class L, int K> struct RecLayout {
@@ -319,6 +333,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     constexpr int TILE_G = TS / W;                 // records per tile
     constexpr int NSUB = TILE_G / 32;              // sub-tiles of 32 records
     constexpr int NWARP = BLOCK / 32;
+    constexpr int kUnroll = IS_F64 ? RPY_SYM_UNROLL_F64 : RPY_SYM_UNROLL_F32;
     constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
     static_assert(TILE_G % 32 == 0 && R::LEN * sizeof(S) == 48, "record geometry");
 
@@ -398,7 +413,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
             const int q = (p + warp * (NSUB / NWARP > 0 ? NSUB / NWARP : 1)) % NSUB;
             const S* sub = tile + (q * 32) * R::LEN;
             V uj[3] = {L::bc(0.0), L::bc(0.0), L::bc(0.0)};
-#pragma unroll (IS_F64 ? 2 : 4)     // measured: fp32 880 -> 896 G pairs/s with 4, fp64 best with 2
+#pragma unroll kUnroll              // measured (cfg 3): fp32 881 / 897 / 899 G pairs/s with 2 / 4 / 8; fp64 374 / 381 / 387 with 1 / 2 / 4
             for (int s = 0; s < 32; ++s) {
                 const int g = (s + lane) & 31;
                 const V* r = reinterpret_cast<const V*>(sub + g * R::LEN);
