@@ -17,7 +17,7 @@ CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "librpy_matvec.so"
 SOURCES = [CSRC / "rpy_matvec.cu", CSRC / "rpy_rigid.cu"]
-DEPS = SOURCES + [CSRC / "rpy_math.cuh", CSRC / "rpy_kernels.cuh", CSRC / "rpy_internal.h",
+DEPS = SOURCES + [CSRC / "rpy_math.cuh", CSRC / "rpy_kernels.cuh", CSRC / "rpy_launch.cuh", CSRC / "rpy_internal.h",
                INCLUDE / "rpy_matvec.h", INCLUDE / "rpy_rigid.h"]
 
 NVCC_FLAGS = [

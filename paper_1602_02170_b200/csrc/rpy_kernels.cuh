@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "rpy_math.cuh"
+#include "rpy_launch.cuh"
 
 #ifndef RPY_SYM_UNROLL_F32
 #define RPY_SYM_UNROLL_F32 4      // inner-loop unroll of the symmetric kernel (measured)
@@ -53,6 +54,7 @@ __global__ void prepack_kernel(const typename L::S* __restrict__ pos,
 {
     using S = typename L::S;
     using R = RecLayout<L, K>;
+    pdl_enter();
     if (skip != nullptr && *skip != 0) return;      // a caller that enqueues ahead of a device-side decision (rpy_rigid.cu)
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_padded) return;
@@ -90,6 +92,7 @@ __global__ void prepack_targets_kernel(const typename L::S* __restrict__ pos, ty
 {
     using S = typename L::S;
     using R = RecLayout<L, K>;
+    pdl_enter();
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_targets) return;
     S* r = rec + (j / R::W) * R::LEN;
@@ -152,6 +155,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
     static_assert(TILE_G % FLUSH_G == 0, "flush period must divide the tile");
+    pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
 
@@ -329,6 +333,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     constexpr int W = L::W;
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr int TS = BLOCK * T;                  // blobs per tile
+    pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     constexpr int TILE_G = TS / W;                 // records per tile
     constexpr int NSUB = TILE_G / 32;              // sub-tiles of 32 records
@@ -492,6 +497,7 @@ __global__ void finalise_kernel(const double* __restrict__ partial, S* __restric
                                 int64_t row_count3, int64_t vel_rhs_stride, double scale,
                                 const int* __restrict__ skip)
 {
+    pdl_enter();
     int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= per_chunk || (skip != nullptr && *skip != 0)) return;
     // four interleaved running sums (fixed assignment chunk -> sum, fixed final order): the loads of

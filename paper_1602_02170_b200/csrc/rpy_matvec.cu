@@ -174,8 +174,8 @@ cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typen
                             int64_t row_begin, int64_t rows, cudaStream_t st, const int* skip)
 {
     dim3 grid((unsigned)p.n_target_tiles, (unsigned)p.n_chunks);
-    allpairs_fn<L, K, WALL, T>()<<<grid, kBlock, allpairs_smem<L, K>(), st>>>(rec, trec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk, skip);
-    return cudaGetLastError();
+    return rpy::launch_pdl(allpairs_fn<L, K, WALL, T>(), grid, dim3(kBlock), allpairs_smem<L, K>(), st,
+                           rec, trec, partial, row_begin, rows, p.n_tiles, p.tiles_per_chunk, skip);
 }
 
 // Symmetric path (rpy::allpairs_sym_kernel): one right-hand side, all rows, enough tiles.
@@ -234,15 +234,17 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
     dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
     if (p.tile == kSymTile) {
         size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
-        if (wall) rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
-        else      rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB><<<grid, kBlock, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
-    } else {
-        constexpr int B2 = kBlock / 2;
-        size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
-        if (wall) rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
-        else      rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB><<<grid, B2, smem, st>>>(rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+        if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
+                                         rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+        return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
+                               rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
     }
-    return cudaGetLastError();
+    constexpr int B2 = kBlock / 2;
+    size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
+    if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
+                                     rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+    return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
+                           rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
 }
 
 template <class L, int K>
@@ -265,8 +267,8 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         S* tr = reinterpret_cast<S*>(ws + at);
         at += records_bytes(prec, rows, K);
         int threads = 256;
-        rpy::prepack_targets_kernel<L, K><<<(unsigned)((rows + threads - 1) / threads), threads, 0, st>>>(tpos, tr, rows, 1.0 / a);
-        cudaError_t e0 = cudaGetLastError();
+        cudaError_t e0 = rpy::launch_pdl(rpy::prepack_targets_kernel<L, K>, dim3((unsigned)((rows + threads - 1) / threads)), dim3(threads), 0, st,
+                                         tpos, tr, rows, 1.0 / a);
         if (e0 != cudaSuccess) return e0;
         trec = tr;
     }
@@ -282,9 +284,9 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     {
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
-        rpy::prepack_kernel<L, K><<<(unsigned)blocks, threads, 0, st>>>(pos, force, rec, n, n_padded,
-                                                                      force_stride3, 1.0 / a, gacc, sym ? n * 3 : 0, skip);
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        e = rpy::launch_pdl(rpy::prepack_kernel<L, K>, dim3((unsigned)blocks), dim3(threads), 0, st,
+                            pos, force, rec, n, n_padded, force_stride3, 1.0 / a, gacc, sym ? n * 3 : (int64_t)0, skip);
+        if (e != cudaSuccess) return e;
     }
     if (sym) {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
@@ -313,11 +315,10 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
             return cudaSuccess;
         }
         (void)vel_stride3;
-        if (vel_f64) rpy::finalise_kernel<double><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<double*>(vel), per_chunk, n_slices,
-                                                                                     rows * 3, vel_stride3, scale, skip);
-        else         rpy::finalise_kernel<S><<<(unsigned)blocks, threads, 0, st>>>(partial, static_cast<S*>(vel), per_chunk, n_slices,
-                                                                               rows * 3, vel_stride3, scale, skip);
-        e = cudaGetLastError();
+        if (vel_f64) e = rpy::launch_pdl(rpy::finalise_kernel<double>, dim3((unsigned)blocks), dim3(threads), 0, st,
+                                         partial, static_cast<double*>(vel), per_chunk, n_slices, rows * 3, vel_stride3, scale, skip);
+        else         e = rpy::launch_pdl(rpy::finalise_kernel<S>, dim3((unsigned)blocks), dim3(threads), 0, st,
+                                         partial, static_cast<S*>(vel), per_chunk, n_slices, rows * 3, vel_stride3, scale, skip);
     }
     return e;
 }

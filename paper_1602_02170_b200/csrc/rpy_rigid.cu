@@ -16,6 +16,7 @@
 #include <stddef.h>
 #include "../../include/rpy_rigid.h"
 #include "rpy_math.cuh"
+#include "rpy_launch.cuh"
 #include "rpy_internal.h"
 
 namespace {
@@ -127,6 +128,7 @@ __global__ void saddle_tail_kernel(const double* __restrict__ pos, const double*
                                    int64_t n_blobs, int64_t n_bodies, int64_t stride, rpy::PartialSums ps,
                                    const int* __restrict__ skip)
 {
+    rpy::pdl_enter();
     const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (skip != nullptr && *skip != 0) return;
@@ -822,6 +824,7 @@ precond_apply_kernel(const void* __restrict__ precond, const double* __restrict_
                      const int* __restrict__ skip)
 {
     __shared__ double red[WPB > 1 ? WPB : 1][128];
+    rpy::pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t p = (int64_t)blockIdx.x * (4 / WPB) + warp / WPB;
@@ -970,6 +973,7 @@ __global__ void __launch_bounds__(kVecThreads)
 dots_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, const double* __restrict__ w, int64_t n,
             double* __restrict__ partial, int pvec, const int* __restrict__ skip)
 {
+    rpy::pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     int64_t lo, hi; chunk_of(n, lo, hi);
     chunk_dots(V, ldv, nrhs, nvec, w + (int64_t)blockIdx.y * ldv, lo, hi, partial, pvec);
@@ -1056,6 +1060,7 @@ update_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, dou
     __shared__ double red[kVecThreads / 32];
     __shared__ double stage[RPY_RIGID_MAX_BATCH][3 * (RPY_RIGID_MAX_RESTART + 2)];
     __shared__ int s_last;
+    rpy::pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     const int r = blockIdx.y;
     for (int v = threadIdx.x >> 5; v < nvec; v += kVecThreads / 32) {      // one warp per dot product
@@ -1135,6 +1140,7 @@ update_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int nvec, dou
 // cleared.  The cycle's stop flag is cleared.
 __global__ void cycle_start_kernel(GmresState st, const double* __restrict__ norm_partial, int nblk, int set_bnorm)
 {
+    rpy::pdl_enter();
     const int r = blockIdx.x, ldr = st.restart + 1;
     double s = 0.0;
     for (int b = threadIdx.x; b < nblk; b += 32) s += norm_partial[(int64_t)r * nblk + b];
@@ -1156,6 +1162,7 @@ __global__ void cycle_start_kernel(GmresState st, const double* __restrict__ nor
 // already solved exactly, or a zero right-hand side) gives y_i = 0.
 __global__ void solve_y_kernel(GmresState st, int k)
 {
+    rpy::pdl_enter();
     if (threadIdx.x != 0) return;
     const int r = blockIdx.x, m = st.restart, ldr = m + 1;
     const double* R = st.R + (int64_t)r * ldr * m; const double* g = st.g + (int64_t)r * ldr;
@@ -1172,6 +1179,7 @@ __global__ void solve_y_kernel(GmresState st, int k)
 __global__ void combine_kernel(const double* __restrict__ V, int64_t ldv, int nrhs, int k, const double* __restrict__ y,
                                int ylen, double* __restrict__ out, int64_t n)
 {
+    rpy::pdl_enter();
     const int r = blockIdx.y;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         double s = 0.0;
@@ -1184,6 +1192,7 @@ __global__ void combine_kernel(const double* __restrict__ V, int64_t ldv, int nr
 __global__ void axpby_kernel(double alpha, const double* __restrict__ x, int64_t x_stride, double beta,
                              double* __restrict__ y, int64_t y_stride, int64_t n)
 {
+    rpy::pdl_enter();
     const double* xr = x + (int64_t)blockIdx.y * x_stride; double* yr = y + (int64_t)blockIdx.y * y_stride;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
         yr[i] = beta == 0.0 ? alpha * xr[i] : alpha * xr[i] + beta * yr[i];
@@ -1194,6 +1203,7 @@ __global__ void __launch_bounds__(kVecThreads)
 norm_partial_kernel(const double* __restrict__ w, int64_t ldv, int64_t n, double* __restrict__ norm_partial)
 {
     __shared__ double red[kVecThreads / 32];
+    rpy::pdl_enter();
     const double* wr = w + (int64_t)blockIdx.y * ldv;
     int64_t lo, hi; chunk_of(n, lo, hi);
     double nrm = 0.0;
@@ -1211,6 +1221,7 @@ norm_partial_kernel(const double* __restrict__ w, int64_t ldv, int64_t n, double
 __global__ void to_float_kernel(const double* __restrict__ in, int64_t in_stride, float* __restrict__ out, int64_t out_stride, int64_t n,
                                 const int* __restrict__ skip = nullptr)
 {
+    rpy::pdl_enter();
     if (skip != nullptr && *skip != 0) return;
     const double* a = in + (int64_t)blockIdx.y * in_stride; float* o = out + (int64_t)blockIdx.y * out_stride;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) o[i] = (float)a[i];
@@ -1344,7 +1355,8 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
 {
     rpy_status s;
     const bool f64 = prec == RPY_PREC_F64;
-    if (!f64 && !lam32_ready) to_float_kernel<<<vgrid(nrhs), 256, 0, st>>>(in, stride, W.lam32, 3 * N, 3 * N, skip);
+    if (!f64 && !lam32_ready)
+        RPY_CUDA_TRY(rpy::launch_pdl(to_float_kernel, vgrid(nrhs), dim3(256), 0, st, in, stride, W.lam32, 3 * N, 3 * N, skip));
     const void* mpos = f64 ? (const void*)pos : (const void*)W.pos32;
     const void* mforce = f64 ? (const void*)in : (const void*)W.lam32;
     const int64_t fstride = f64 ? stride : 3 * N;
@@ -1356,21 +1368,21 @@ rpy_status saddle(int wall, rpy_prec prec, int64_t N, int64_t nb, const double* 
                                 skip, nullptr, sh.shard, sh.n_shards, true);
         if (s != RPY_OK) return s;
         if (sh.reduce(sh.ctx, out, 3 * N, st) != 0) return RPY_ERR_ARG;
-        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(saddle_tail_kernel, bg, dim3(128), 0, st, pos, q, off, in, (const float*)nullptr, out, N, nb, stride, ps, skip));
     } else if (nrhs == 1 || nrhs == 2 || nrhs == 4 || nrhs == 8) {
         // one right-hand-side group: the product stops before its finalise step, the tail adds the slices
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, mpos, mforce, fstride, nullptr, 0, a, eta, W.mv, W.mv_bytes, st,
                                 skip, &ps);
         if (s != RPY_OK) return s;
-        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(saddle_tail_kernel, bg, dim3(128), 0, st, pos, q, off, in, (const float*)nullptr, out, N, nb, stride, ps, skip));
     } else if (f64) {
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, pos, in, stride, out, stride, a, eta, W.mv, W.mv_bytes, st, skip);
         if (s != RPY_OK) return s;
-        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, nullptr, out, N, nb, stride, ps, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(saddle_tail_kernel, bg, dim3(128), 0, st, pos, q, off, in, (const float*)nullptr, out, N, nb, stride, ps, skip));
     } else {
         s = rpy::matvec_strided(wall != 0, prec, N, nrhs, W.pos32, W.lam32, 3 * N, W.vel32, 3 * N, a, eta, W.mv, W.mv_bytes, st, skip);
         if (s != RPY_OK) return s;
-        saddle_tail_kernel<<<bg, 128, 0, st>>>(pos, q, off, in, W.vel32, out, N, nb, stride, ps, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(saddle_tail_kernel, bg, dim3(128), 0, st, pos, q, off, in, (const float*)W.vel32, out, N, nb, stride, ps, skip));
     }
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
@@ -1384,11 +1396,11 @@ rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const doubl
     // one warp per body streams the inverses at HBM speed once there are enough bodies; below that four warps
     // per body (a CTA each) keep more loads in flight
     if (nb >= 8192)
-        precond_apply_kernel<1><<<dim3(warp_grid(nb, 128), (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32,
-                                                                                        scal, vnorm, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(precond_apply_kernel<1>, dim3(warp_grid(nb, 128), (unsigned)nrhs), dim3(128), 0, st,
+                                     precond, in, out, N, nb, stride, lam32, scal, vnorm, skip));
     else
-        precond_apply_kernel<4><<<dim3((unsigned)nb, (unsigned)nrhs), 128, 0, st>>>(precond, in, out, N, nb, stride, lam32,
-                                                                                  scal, vnorm, skip);
+        RPY_CUDA_TRY(rpy::launch_pdl(precond_apply_kernel<4>, dim3((unsigned)nb, (unsigned)nrhs), dim3(128), 0, st,
+                                     precond, in, out, N, nb, stride, lam32, scal, vnorm, skip));
     RPY_CUDA_TRY(cudaGetLastError());
     return RPY_OK;
 }
@@ -1717,12 +1729,12 @@ rpy_status solve_batch(int wall, rpy_prec matvec_prec, int64_t N, int64_t nb, in
         if (e != RPY_OK) return e;
         // classical Gram-Schmidt, twice (as accurate as the modified form; three launches for the two passes)
         StepEnd ej = end; ej.j = j;
-        dots_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, ctl);
-        update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial, pvec, W.st.hcol, 0, W.norm_partial,
-                                                 W.partial2, W.st, no_end, ctl);
-        update_kernel<<<vg, kVecThreads, 0, st>>>(W.V, ldv, nrhs, j + 1, W.w, n, W.partial2, pvec, W.st.hcol, 1, W.norm_partial,
-                                                 nullptr, W.st, ej, ctl);
-        RPY_CUDA_TRY(cudaGetLastError());
+        const dim3 vt(kVecThreads);
+        RPY_CUDA_TRY(rpy::launch_pdl(dots_kernel, vg, vt, 0, st, (const double*)W.V, ldv, nrhs, j + 1, (const double*)W.w, n, W.partial, pvec, ctl));
+        RPY_CUDA_TRY(rpy::launch_pdl(update_kernel, vg, vt, 0, st, (const double*)W.V, ldv, nrhs, j + 1, W.w, n, (const double*)W.partial, pvec,
+                                     W.st.hcol, 0, W.norm_partial, W.partial2, W.st, no_end, ctl));
+        RPY_CUDA_TRY(rpy::launch_pdl(update_kernel, vg, vt, 0, st, (const double*)W.V, ldv, nrhs, j + 1, W.w, n, (const double*)W.partial2, pvec,
+                                     W.st.hcol, 1, W.norm_partial, (double*)nullptr, W.st, ej, ctl));
         return RPY_OK;
     };
 
