@@ -521,7 +521,7 @@ def run_ours(args):
             achieved = pairs_launch * fl / (k_ms * 1e-3) / 1e12
             peak = peak_tflops(p)
             lane_peak = SM_COUNT * LANES[p] * SM_MAX_GHZ * 1e9
-            traffic, src = ncu_traffic(cfg, p, v) if w.n_rhs == 1 else (None, None)
+            traffic, src = ncu_traffic(cfg, p, v) if w.n_rhs == 1 else (None, None)   # captures exist for k = 1
             return {
                 "bound": "alu", "kernel": "allpairs_sym_kernel" if plan_["symmetric"] else "allpairs_kernel",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
