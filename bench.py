@@ -19,6 +19,9 @@ pair-RHS products N^2 k / t are in "pair_rhs_gps").
   roofline  ALU bound: algorithmic flops of the all-pairs kernel / its CUDA-event duration,
             against 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (fp64: 64 lanes), DESIGN.md
   cpu_baseline  the float64 oracle (oracle/) on this box's host cores, on a bounded row sample
+  parity    rel-L2 and per-blob maximum error of the timed step's result against that oracle sample
+            (exit status 3 when outside north_star's tolerance)
+  value_f64, roofline_f64, parity_f64   the fp64 path on the same workload (the paper's precision)
 
 N > 1 (torchrun): the work is sharded across ranks -- one right-hand side: each rank takes 1/N of the
 unordered tile pairs of the symmetric kernel and one NCCL all-reduce adds the partial u; several

@@ -810,7 +810,7 @@ __global__ void precond_finish_kernel(const int* __restrict__ info, int64_t n_bo
 // instead of waiting on 2m dependent substitution steps.
 // WPB warps per body (CTA of 128 threads = 4 / WPB bodies): with WPB = 4 each warp takes a quarter of the
 // columns and the four partial sums are added through shared memory in a fixed order -- four times as many
-// loads in flight when there are too few bodies to fill the GPU with one warp each.
+// loads in flight when there are too few bodies (< 2,048) to fill the GPU with one warp each.
 // With `vnorm` set the input is first scaled, v = scal[rhs][1] * in (the Arnoldi normalisation v_{j+1} = w / h_{j+1,j},
 // or r / beta at the start of a cycle), v is stored to vnorm as the new Krylov vector and the kernel applies P^-1
 // to it: the normalisation costs no launch of its own.
@@ -1393,9 +1393,10 @@ rpy_status precond_apply(int64_t N, int64_t nb, const void* precond, const doubl
                          int nrhs, cudaStream_t st, float* lam32 = nullptr, const double* scal = nullptr,
                          double* vnorm = nullptr, const int* skip = nullptr)
 {
-    // one warp per body streams the inverses at HBM speed once there are enough bodies; below that four warps
-    // per body (a CTA each) keep more loads in flight
-    if (nb >= 8192)
+    // one warp per body streams the inverses at HBM speed once there are enough bodies (cfg 3, 4,096 bodies:
+    // 0.099 ms = 5.9 TB/s against 0.120 ms with four); below ~14 warps per SM four warps per body (a CTA each)
+    // keep more loads in flight (cfg 2, 1,000 bodies: 14 against 30 us cold)
+    if (nb >= 2048)
         RPY_CUDA_TRY(rpy::launch_pdl(precond_apply_kernel<1>, dim3(warp_grid(nb, 128), (unsigned)nrhs), dim3(128), 0, st,
                                      precond, in, out, N, nb, stride, lam32, scal, vnorm, skip));
     else

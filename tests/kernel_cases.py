@@ -110,8 +110,8 @@ def case_precond_all_paths():
     U = torch.randn(db.n_bodies, 6, dtype=torch.float64, device="cuda")
     finite(rigid.rpy_rigid_K_apply(db, U), "K")
     finite(rigid.rpy_rigid_KT_apply(db, torch.randn(db.n_blobs, 3, dtype=torch.float64, device="cuda")), "KT")
-    # one warp per body needs >= 8,192 bodies: single blobs
-    n = 8200
+    # one warp per body needs >= 2,048 bodies: single blobs
+    n = 2100
     rng = np.random.default_rng(3)
     p1 = np.column_stack([rng.uniform(0, 900, n), rng.uniform(0, 900, n), rng.uniform(1.5, 4, n)])
     d1 = rigid.bodies(dev(p1), dev(p1), np.arange(n + 1))
