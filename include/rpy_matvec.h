@@ -186,8 +186,8 @@ rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void *d_po
  *     M_ij = M_ji^T to build every unordered pair's coefficients once.  Blobs are
  *     cut into tiles of *tile_sources (= *targets_per_cta: 128 below 50,000 blobs, else 256); a CTA owns one tile I and walks the
  *     tiles (I + d) mod n_tiles for one of *n_source_chunks chunks of the distances d = 0..n_tiles/2.
- *     The transposed half of the sum is accumulated with fp64 atomics, so the result is
- *     reproducible to rounding of the double sums (~1e-16 relative), not bit for bit; the plain
+ *     Both halves of every CTA's work are accumulated with fp64 atomics into one double array, so the
+ *     result is reproducible to rounding of the double sums (~1e-16 relative), not bit for bit; the plain
  *     kernel (and therefore every *_rows call and every n_rhs > 1 call) is bit-reproducible.
  *   *n_ctas: CTAs of the launch. */
 rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int64_t row_count,

@@ -323,7 +323,7 @@ template <> __device__ __forceinline__ double lane_elem<float2>(float2 v, int w)
 
 template <class L, bool WALL, int T, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
-allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ partial, double* __restrict__ gacc,
+allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ gacc,
                     int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end,
                     const int* __restrict__ skip)
 {
@@ -476,14 +476,15 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
         }
     }
 
-    double* out = partial + (int64_t)blockIdx.y * n_blobs * 3;
+    // the forward half of this CTA's chunk joins the transposed halves in the one double accumulator: no per-chunk
+    // slices to write and to add up afterwards (at N = 15,000 they were 61 x 360 KB per product)
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        if (row[t] < n_blobs) {
+        if (row[t] < n_blobs && my_tiles > 0) {
 #pragma unroll
             for (int c = 0; c < 3; ++c)
-                if constexpr (IS_F64) out[row[t] * 3 + c] = L::hsum(acc[t][c]);
-                else                  out[row[t] * 3 + c] = dacc[t][c];
+                if constexpr (IS_F64) atomicAdd(gacc + row[t] * 3 + c, L::hsum(acc[t][c]));
+                else                  atomicAdd(gacc + row[t] * 3 + c, dacc[t][c]);
         }
     }
 }

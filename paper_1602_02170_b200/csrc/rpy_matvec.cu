@@ -206,6 +206,7 @@ SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
     SymPlan p;
     // Tiles of 256 blobs (128 threads x 2 targets) once there are enough of them to fill the chip several
     // times over; 128-blob tiles (64 threads x 2) below that: four times as many, four times smaller CTAs.
+    // (64-blob tiles, one warp per CTA, were measured too: a gain only at N = 3,584 ... 3,900)
     p.tile = n < RPY_SYM_SMALL_BELOW ? kSymTile / 2 : kSymTile;
     p.n_padded = (n + kSymTile - 1) / kSymTile * kSymTile;       // records are padded to 256 either way
     p.nt = (int)((n + p.tile - 1) / p.tile);
@@ -227,7 +228,7 @@ template <> struct SymShape<rpy::Lane<float2>> { static constexpr int MINB = RPY
 template <> struct SymShape<rpy::Lane<double>> { static constexpr int MINB = RPY_SYM_MINB_F64; };
 
 template <class L>
-cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, double* partial, double* gacc,
+cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, double* gacc,
                        int64_t n, cudaStream_t st, const int* skip)
 {
     constexpr int MINB = SymShape<L>::MINB;
@@ -235,16 +236,16 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
     if (p.tile == kSymTile) {
         size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
         if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
-                                         rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                                         rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
         return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
-                               rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                               rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
     }
     constexpr int B2 = kBlock / 2;
     size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
     if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
-                                     rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                                     rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
     return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
-                           rec, partial, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                           rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
 }
 
 template <class L, int K>
@@ -279,8 +280,8 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
     cudaError_t e;
     int n_slices = p.n_chunks;
-    // slice n_chunks of `partial` receives the symmetric kernel's transposed half through fp64 atomics
-    double* gacc = sym ? partial + (int64_t)sp.n_chunks * n * 3 : nullptr;
+    // symmetric kernel: ONE slice, which receives both halves of every CTA's work through fp64 atomics
+    double* gacc = sym ? partial : nullptr;
     {
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
@@ -290,9 +291,9 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     }
     if (sym) {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
-        if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, partial, gacc, n, st, skip);
+        if constexpr (K == 1) e = launch_sym<L>(wall, sp, rec, gacc, n, st, skip);
         else e = cudaErrorInvalidValue;
-        n_slices = sp.n_chunks + 1;
+        n_slices = 1;
     } else {
         if (ev && (e = cudaEventRecord(static_cast<cudaEvent_t>(ev[1]), st)) != cudaSuccess) return e;
         constexpr int T2 = K <= 2 ? 2 : 1;     // choose_T never asks for T = 2 when K > 2
