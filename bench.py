@@ -310,7 +310,9 @@ def time_config(torch, binding, wl, prec, variant, steps, warmup, flush_buf, ran
         dist.all_reduce(total, op=dist.ReduceOp.MAX)
     ms_per_step = total.item() / steps
     return {"ms_per_step": ms_per_step, "ms_min": min(ms), "gps": n * n / (ms_per_step * 1e-3) / 1e9,
-            "pos": pos, "force": force, "ws": ws, "out": out if world == 1 else None}
+            "pos": pos, "force": force, "ws": ws,
+            # the full u: single GPU, or after the all-reduce of the work shards (every rank holds it)
+            "out": out if (world == 1 or work_shards) else None}
 
 
 def time_allpairs_kernel(torch, binding, res, wl, variant, steps, flush_buf):
@@ -548,6 +550,9 @@ def run_ours(args):
             gps, cores, desc, t, _, orows, oref = oracle_sample(wl, variant, prec, 15.0)
             cpu = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
             parity = parity_of(res["out"], oref, orows, prec)
+        elif world > 1 and res["out"] is not None and not args.no_cpu:
+            parity = oracle_parity(wl, variant, prec, res["out"])      # the all-reduced sum of the ranks' shards
+        if parity is not None:
             parity_failed = parity_failed or not parity["ok"]
             log(f"[bench] parity vs oracle: {parity}")
         line = {
