@@ -311,3 +311,31 @@ def test_work_shards_sum_to_the_full_product(prec, variant, n_bodies, n_shards, 
     check(total.cpu().numpy(), ref, prec, f"shards n={w.n_blobs} G={n_shards} {variant}")
     one = fn(pos, lam, 0, 1)                          # a single shard is the whole product
     check(one.cpu().numpy().astype(np.float64), ref, prec, "single shard")
+
+
+@pytest.mark.parametrize("n", [2000, 6000])
+def test_product_is_capturable_in_a_cuda_graph(n):
+    """The device forms allocate nothing, create no CUDA object and never synchronise (include/rpy_matvec.h), so a
+    caller can capture the whole product -- three kernels chained by programmatic dependent launch -- in a CUDA
+    graph and replay it; plain (n = 2,000) and symmetric (n = 6,000) kernel.  The replay on new inputs equals the
+    eager call."""
+    w = workloads.config1(seed=3, n=n)
+    pos = torch.from_numpy(w.pos).cuda(); lam = torch.from_numpy(w.force).cuda()
+    ws = torch.empty(binding.rpy_matvec_workspace_bytes("f64", n, 1), dtype=torch.uint8, device="cuda")
+    out = torch.empty_like(lam)
+    binding.rpy_wall_matvec(pos, lam, out=out, workspace=ws)            # loads the module before capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            binding.rpy_wall_matvec(pos, lam, out=out, workspace=ws)
+    lam2 = torch.from_numpy(np.random.default_rng(9).standard_normal(w.force.shape)).cuda()
+    lam.copy_(lam2)                                                     # new forces in the captured buffers
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    eager = binding.rpy_wall_matvec(pos, lam2)
+    assert float((out - eager).norm() / eager.norm()) <= 1e-14
+    ref = oracle.matvec(oracle.WALL, w.pos, lam2.cpu().numpy())
+    check(out.cpu().numpy(), ref, "f64", f"graph replay n={n}")
