@@ -433,15 +433,32 @@ def size_sweep(torch):
         for prec, dt in (("f32", torch.float32), ("f64", torch.float64)):
             pos = torch.from_numpy(w.pos).to(dt).cuda(); lam = torch.from_numpy(w.force).to(dt).cuda()
             plan = binding.rpy_matvec_launch_plan(prec, n, 1, n)
-            ts = []
+            ts, ts_all = [], []
             for _ in range(8):
                 _, ev = bench_aids.matvec_phases("wall", pos, lam)
                 torch.cuda.synchronize()
-                ts.append((ev[1].elapsed_time(ev[2]), ev[0].elapsed_time(ev[3])))
-            k_ms = min(t[0] for t in ts[2:]); tot = min(t[1] for t in ts[2:])
+                ts.append(ev[1].elapsed_time(ev[2])); ts_all.append(ev[0].elapsed_time(ev[3]))
+            k_ms = min(ts[2:])
+            ph_ms = min(t for t in ts_all[2:])               # prepack .. finalise with events between the kernels (as in r1g)
+            # the product as the device sees it: ten back-to-back products captured in a CUDA graph (no host work,
+            # no events between its kernels -- they would undo the programmatic dependent launch), replayed
+            ws = torch.empty(binding.rpy_matvec_workspace_bytes(prec, n, 1), dtype=torch.uint8, device=pos.device)
+            out = torch.empty_like(lam)
+            g = torch.cuda.CUDAGraph(); side = torch.cuda.Stream()
+            torch.cuda.synchronize()
+            with torch.cuda.stream(side):
+                with torch.cuda.graph(g, stream=side):
+                    for _ in range(10):
+                        binding.rpy_wall_matvec(pos, lam, out=out, workspace=ws)
+            tot = 1e9
+            for _ in range(4):
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(); g.replay(); e1.record(); torch.cuda.synchronize()
+                tot = min(tot, e0.elapsed_time(e1) / 10)
+            del g
             ops, _ = work_per_pair(prec, "wall", 1, plan["symmetric"])
             rows.append({"n": n, "prec": prec, "symmetric": plan["symmetric"], "tile": plan["tile_sources"],
-                         "n_ctas": plan["n_ctas"], "kernel_us": k_ms * 1e3, "product_us": tot * 1e3,
+                         "n_ctas": plan["n_ctas"], "kernel_us": k_ms * 1e3, "product_us": tot * 1e3, "product_phases_us": ph_ms * 1e3,
                          "gps_kernel": n * n / k_ms / 1e6, "pipe_frac": n * n * ops / (k_ms * 1e-3) / lane[prec]})
             log(f"[sweep] {rows[-1]}")
     return rows

@@ -155,7 +155,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
     static_assert(TILE_G % FLUSH_G == 0, "flush period must divide the tile");
-    pdl_enter();
+    pdl_wait();
     if (skip != nullptr && *skip != 0) return;
     static_assert(TILE_BYTES % 16 == 0, "bulk copy size");
 
@@ -333,7 +333,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     constexpr int W = L::W;
     constexpr bool IS_F64 = sizeof(S) == 8;
     constexpr int TS = BLOCK * T;                  // blobs per tile
-    pdl_enter();
+    pdl_wait();
     if (skip != nullptr && *skip != 0) return;
     constexpr int TILE_G = TS / W;                 // records per tile
     constexpr int NSUB = TILE_G / 32;              // sub-tiles of 32 records

@@ -194,6 +194,8 @@ struct Opts {
     bool vel_f64 = false;           // vel is double whatever the path (partial products of a shard)
     const int* skip = nullptr;      // device flag: non-zero turns every kernel of the call into a no-op
     rpy::PartialSums* partials = nullptr;   // non-null: finalise is left to the caller, who gets the slices
+    bool chain_in = false;          // the call's first kernel may be scheduled under the kernel before it in the stream
+                                    // (programmatic dependent launch): a caller that chains its own kernels (the solver)
 };
 
 inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
@@ -268,7 +270,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
         S* tr = reinterpret_cast<S*>(ws + at);
         at += records_bytes(prec, rows, K);
         int threads = 256;
-        cudaError_t e0 = rpy::launch_pdl(rpy::prepack_targets_kernel<L, K>, dim3((unsigned)((rows + threads - 1) / threads)), dim3(threads), 0, st,
+        cudaError_t e0 = rpy::launch_chain(o.chain_in, rpy::prepack_targets_kernel<L, K>, dim3((unsigned)((rows + threads - 1) / threads)), dim3(threads), 0, st,
                                          tpos, tr, rows, 1.0 / a);
         if (e0 != cudaSuccess) return e0;
         trec = tr;
@@ -285,7 +287,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     {
         int threads = 256;
         int64_t blocks = (n_padded + threads - 1) / threads;
-        e = rpy::launch_pdl(rpy::prepack_kernel<L, K>, dim3((unsigned)blocks), dim3(threads), 0, st,
+        e = rpy::launch_chain(o.chain_in || tpos != nullptr, rpy::prepack_kernel<L, K>, dim3((unsigned)blocks), dim3(threads), 0, st,
                             pos, force, rec, n, n_padded, force_stride3, 1.0 / a, gacc, sym ? n * 3 : (int64_t)0, skip);
         if (e != cudaSuccess) return e;
     }
@@ -529,6 +531,7 @@ rpy_status matvec_strided(bool wall, rpy_prec prec, int64_t n, int n_rhs, const 
     Opts o;
     o.vel_stride3 = partials ? 3 * n : vel_stride3; o.force_stride3 = force_stride3;
     o.skip = d_skip; o.partials = partials; o.sh = Shard{shard, n_shards}; o.vel_f64 = vel_f64;
+    o.chain_in = true;                            // internal callers launch their own kernels chained as well
     cudaError_t e = prec == RPY_PREC_F64
         ? run_all_groups<rpy::Lane<double>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o)
         : run_all_groups<rpy::Lane<float2>>(wall, n, n_rhs, 0, n, d_pos, d_force, d_vel, a, eta, ws, st, nullptr, nullptr, o);
