@@ -606,7 +606,7 @@ def run_ours(args):
         # --- the other BASELINE.json configurations, fewer steps (context; not the headline)
         if world == 1 and not args.no_extra:
             extra = []
-            for cfg, p, v, st in ((5, "f32", "wall", 3), (5, "f32", "free", 3),
+            for cfg, p, v, st in ((3, "f32", "free", 3), (3, "f64", "free", 3), (5, "f32", "wall", 3), (5, "f32", "free", 3),
                                   (2, "f64", "wall", 10), (2, "f32", "wall", 10), (1, "f64", "wall", 10),
                                   (4, "f32", "wall", 1), (3, "f64", "wall", 3)):
                 if (cfg, p, v) == (args.config, prec, variant) or ((cfg, v) == (args.config, variant) and "value_f64" in line and p == "f64"):

@@ -80,24 +80,31 @@ rpy_status rpy_rigid_KT_apply(int64_t n_blobs, int64_t n_bodies, const double *d
 size_t rpy_rigid_precond_bytes(int64_t n_bodies, const int64_t *h_offsets);
 
 /* Builds the preconditioner: for every body the dense M^(pp) (wall != 0: wall-corrected tensor,
- * else free space -- the "unbounded" preconditioner of Table III), its inverse
- * (Cholesky factorisation, then L^-1 and L^-T L^-1 in place), Y and N~_pp.  One CTA per body; the matrix lives in shared memory when 3*blobs <= 162,
- * else in its slot of d_precond.  h_offsets is read before the call returns.
+ * else free space -- the "unbounded" preconditioner of Table III), its explicit inverse
+ * ("dense matrix inversion"), Y = (M^(pp))^-1 K_p and N~_pp = (K_p^T Y)^+ (a
+ * pseudo-inverse, taken with lengths in units of `a` so that it does not depend on the unit of length).
+ * One CTA per body.  Bodies of up to 42 blobs (3*blobs <= 128): a register-resident block sweep of the
+ * augmented matrix [M K; K^T 0] that yields all three in one pass; larger bodies: Cholesky factorisation,
+ * L^-1 and L^-T L^-1 in place, in shared memory when 3*blobs <= 162, else in the body's slot of d_precond.
+ * h_offsets is read before the call returns.
  * d_precond: device, 256-byte aligned, >= rpy_rigid_precond_bytes().  Synchronises the stream once (after
- * copying the offset tables up, before the build kernel is enqueued); a failed
- * factorisation is recorded in d_precond and reported by rpy_rigid_precond_info / the solve.     */
+ * copying the offset tables up, before the build kernels are enqueued); a body that is not positive definite
+ * is recorded in d_precond (its header names the first one) and reported by rpy_rigid_precond_info / the solve. */
 rpy_status rpy_rigid_precond_build(int wall, int64_t n_blobs, int64_t n_bodies, const double *d_pos,
                                    const double *d_q, const int64_t *h_offsets, double a, double eta,
                                    void *d_precond, size_t precond_bytes, void *cuda_stream);
 
-/* Synchronises the stream and writes to *h_first_bad_body the smallest body index whose
- * factorisation (or 6x6 inversion) failed, or -1.  Returns RPY_ERR_NOT_SPD in the former case.                        */
+/* Copies the header of d_precond down (40 bytes; d_precond is only read), synchronises the stream and writes to
+ * *h_first_bad_body the smallest body index whose factorisation (or 6x6 inversion) failed, or -1.  Returns
+ * RPY_ERR_NOT_SPD in the former case, RPY_ERR_ARG when d_precond was not built for n_bodies bodies.          */
 rpy_status rpy_rigid_precond_info(int64_t n_bodies, const void *d_precond, int64_t *h_first_bad_body,
                                   void *cuda_stream);
 
 /* [lambda; U] = P^-1 [x; y]: Eq. (19) for every body.  d_in, d_out: solver vectors
- * (3 n_blobs + 6 n_bodies doubles), d_out must not overlap d_in.  One warp per body:
- * t = (M^(pp))^-1 x (dense symmetric product), U = -N~ (y + Y^T x), lambda = t + Y U.            */
+ * (3 n_blobs + 6 n_bodies doubles), d_out must not overlap d_in.  One warp per body (four below 2,048 bodies):
+ * t = (M^(pp))^-1 x (dense symmetric product), U = -N~ (y + Y^T x), lambda = t + Y U.
+ * No host round trip, so a d_precond that was not built for (n_bodies, n_blobs) cannot be returned as a status:
+ * the kernel then fills d_out with NaN (the solve checks the header on the host and returns RPY_ERR_ARG).  */
 rpy_status rpy_rigid_precond_apply(int64_t n_blobs, int64_t n_bodies, const void *d_precond,
                                    const double *d_in, double *d_out, void *cuda_stream);
 
