@@ -56,9 +56,9 @@ UNIT = "G blob-pairs/s"
 # (MUFU.RSQ64H seed + one cubic Newton step): two roots for the wall tensor, one for free space.
 WORK = {
     # (prec, variant): (lane_ops_geom, lane_ops_per_rhs, flop_geom, flop_per_rhs)
-    ("f32", "wall"): (46, 10, 71, 18),
+    ("f32", "wall"): (44, 10, 70, 18),
     ("f32", "free"): (12, 10, 19, 18),
-    ("f64", "wall"): (54, 10, 83, 18),
+    ("f64", "wall"): (52, 10, 82, 18),
     ("f64", "free"): (17, 10, 24, 18),
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel come from the committed

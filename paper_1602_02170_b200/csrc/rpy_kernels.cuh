@@ -234,26 +234,22 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
                 }
                 // phase 1 (every pair): separation and the r > 2a scalars of Eq. (9)
                 PairCoef<V> c[T];
-                V rxy2[T], r2[T], f[T], G[T];
+                PairPre<V> pre[T];
                 bool near = false;
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    c[t].dx = L::sub(xi[t], xj);
-                    c[t].dy = L::sub(yi[t], yj);
-                    c[t].dz = L::sub(zi[t], zj);
-                    rpy_far_scalars<L>(c[t].dx, c[t].dy, c[t].dz, rxy2[t], r2[t], f[t], G[t]);
-                    near = near || L::any_le(r2[t], 4.0);
+                    pair_pre<L, WALL>(xi[t], yi[t], zi[t], xj, yj, zj, c[t], pre[t]);
+                    near = near || L::any_le(pre[t].r2, 4.0);
                 }
                 // phase 2 (rare, warp-uniform): some lane has an overlapping pair (r <= 2a) or r = 0
                 if (__any_sync(0xffffffffu, near)) {
 #pragma unroll
-                    for (int t = 0; t < T; ++t) rpy_near_fixup<L>(r2[t], f[t], G[t]);
+                    for (int t = 0; t < T; ++t) rpy_near_fixup<L, WALL>(pre[t].r2, pre[t].n1, pre[t].f, pre[t].G);
                 }
                 // phase 3 (every pair): wall scalars and the product with lambda_j
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    if constexpr (WALL) wall_coef<L>(zi[t], zi2[t], zj, rxy2[t], f[t], G[t], c[t]);
-                    else { c[t].al = f[t]; c[t].be = G[t]; }
+                    pair_post<L, WALL>(zi2[t], zj, pre[t], c[t]);
 #pragma unroll
                     for (int s = 0; s < K; ++s)
                         pair_apply<L, WALL>(c[t], lam[s][0], lam[s][1], lam[s][2],
@@ -293,7 +289,7 @@ allpairs_kernel(const typename L::S* __restrict__ rec, const typename L::S* __re
 // coefficients of the unordered pair {i, j} are built ONCE and applied twice,
 //   u_i += M_ij lambda_j   (forward,    accumulators stay with the thread that owns target i),
 //   u_j += M_ij^T lambda_i (transposed, accumulators TRAVEL with the source),
-// which costs 50 + 2*10 FP-pipe operations per unordered pair instead of 2*(50 + 10).
+// which costs 44 + 2*10 FP-pipe operations per unordered pair instead of 2*(44 + 10).
 //
 // Decomposition.  Blobs are cut into tiles of TS = BLOCK*T; tile I meets tile J = (I + d) mod nt
 // for d = 0 .. nt/2: every unordered tile pair exactly once (for even nt the distance nt/2 is
@@ -425,24 +421,20 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
                 V xj = r[0], yj = r[1], zj = r[2];
                 V lj0 = r[3], lj1 = r[4], lj2 = r[5];
                 PairCoef<V> c[T];
-                V rxy2[T], r2[T], f[T], G[T];
+                PairPre<V> pre[T];
                 bool near = false;
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    c[t].dx = L::sub(xi[t], xj);
-                    c[t].dy = L::sub(yi[t], yj);
-                    c[t].dz = L::sub(zi[t], zj);
-                    rpy_far_scalars<L>(c[t].dx, c[t].dy, c[t].dz, rxy2[t], r2[t], f[t], G[t]);
-                    near = near || L::any_le(r2[t], 4.0);
+                    pair_pre<L, WALL>(xi[t], yi[t], zi[t], xj, yj, zj, c[t], pre[t]);
+                    near = near || L::any_le(pre[t].r2, 4.0);
                 }
                 if (__any_sync(0xffffffffu, near)) {
 #pragma unroll
-                    for (int t = 0; t < T; ++t) rpy_near_fixup<L>(r2[t], f[t], G[t]);
+                    for (int t = 0; t < T; ++t) rpy_near_fixup<L, WALL>(pre[t].r2, pre[t].n1, pre[t].f, pre[t].G);
                 }
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
-                    if constexpr (WALL) wall_coef<L>(zi[t], zi2[t], zj, rxy2[t], f[t], G[t], c[t]);
-                    else { c[t].al = f[t]; c[t].be = G[t]; }
+                    pair_post<L, WALL>(zi2[t], zj, pre[t], c[t]);
                     pair_apply<L, WALL>(c[t], lj0, lj1, lj2, acc[t][0], acc[t][1], acc[t][2]);
                     if constexpr (WALL) { V tmp = c[t].ga; c[t].ga = c[t].ep; c[t].ep = tmp; }   // M^T: xz <-> zx
                     pair_apply<L, WALL>(c[t], lt[t][0], lt[t][1], lt[t][2], uj[0], uj[1], uj[2]);

@@ -261,12 +261,12 @@ __device__ __forceinline__ void pair_block(double xi, double yi, double zi, doub
 {
     using L = rpy::Lane<double>;
     rpy::PairCoef<double> c;
-    c.dx = xi - xj; c.dy = yi - yj; c.dz = zi - zj;
-    double rxy2, r2, f, G;
-    rpy::rpy_far_scalars<L>(c.dx, c.dy, c.dz, rxy2, r2, f, G);
-    if (r2 <= 4.0) rpy::rpy_near_fixup<L>(r2, f, G);
+    rpy::PairPre<double> pre;
+    rpy::pair_pre<L, WALL>(xi, yi, zi, xj, yj, zj, c, pre);
+    if (pre.r2 <= 4.0) rpy::rpy_near_fixup<L, WALL>(pre.r2, pre.n1, pre.f, pre.G);
+    rpy::pair_post<L, WALL>(2.0 * zi, zj, pre, c);
+    const double f = pre.f, G = pre.G;
     if (WALL) {
-        rpy::wall_coef<L>(zi, 2.0 * zi, zj, rxy2, f, G, c);
         B[0] = c.al + c.be * c.dx * c.dx; B[1] = c.be * c.dx * c.dy;        B[2] = c.ga * c.dx;
         B[3] = B[1];                      B[4] = c.al + c.be * c.dy * c.dy; B[5] = c.ga * c.dy;
         B[6] = c.ep * c.dx;               B[7] = c.ep * c.dy;               B[8] = c.de;

@@ -38,11 +38,11 @@ def pytest_approx(x):
 
 
 def test_work_model_matches_the_expression_tree_counts():
-    # wall 46 + 10k lane-ops per ordered pair (plain), (46 + 20k) / 2 symmetric; fp64 adds the roots
-    assert bench.work_per_pair("f32", "wall", 1) == (56, 89)
-    assert bench.work_per_pair("f32", "wall", 8) == (126, 215)
-    assert bench.work_per_pair("f32", "wall", 1, symmetric=True) == (33.0, 53.5)
-    assert bench.work_per_pair("f64", "wall", 1, symmetric=True) == (37.0, 59.5)
+    # wall 44 + 10k lane-ops per ordered pair (plain), (44 + 20k) / 2 symmetric; fp64 adds the roots
+    assert bench.work_per_pair("f32", "wall", 1) == (54, 88)
+    assert bench.work_per_pair("f32", "wall", 8) == (124, 214)
+    assert bench.work_per_pair("f32", "wall", 1, symmetric=True) == (32.0, 53.0)
+    assert bench.work_per_pair("f64", "wall", 1, symmetric=True) == (36.0, 59.0)
     assert bench.work_per_pair("f32", "free", 1, symmetric=True) == (16.0, 27.5)
     assert abs(bench.peak_tflops("f32") - 74.45) < 0.01 and abs(bench.peak_tflops("f64") - 37.22) < 0.01
 
