@@ -528,6 +528,11 @@ def run_ours(args):
         try:
             for kind, name in ((0, "ffma"), (1, "ffma2"), (2, "dfma"), (3, "mufu_rsq"), (4, "ffma2_three_reg"), (5, "ffma_three_reg")):
                 probe[name + "_g_per_s"] = round(bench_aids.pipe_probe(kind, 8192)["gfma_per_s"], 1)
+            # what an FFMA2 / DFMA costs by operand form (T lane-ops/s at 4 CTAs x 128 threads per SM): the all-pairs
+            # kernels are bound by register-operand delivery, DESIGN.md section 6
+            probe["operand_forms_tlaneops_per_s"] = {
+                bench_aids.OPERAND_FORMS[kind]: round(bench_aids.operand_probe(kind, 4, 8192)["tlaneops_per_s"], 2)
+                for kind in range(8)}
         except Exception as e:  # pragma: no cover
             probe = {"error": str(e)}
 

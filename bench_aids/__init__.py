@@ -3,6 +3,7 @@
     python -m bench_aids [--force]      builds bench_aids/librpy_bench_aids.so with nvcc for sm_100a
 
 * ``pipe_probe``      FMA-chain rates of the FP32 / FP64 / MUFU pipes (the ALU roofline's denominator)
+* ``operand_probe``   what an FFMA2 / DFMA costs by the form of its operands (register pairs, reuse, scalar, immediate)
 * ``coissue_probe``   DFMA chains beside FFMA2 chains on every SM
 * ``matvec_phases``   the product (``librpy_matvec.so``) with CUDA events around each of its kernels
 
@@ -68,6 +69,8 @@ def load_library(rebuild: bool = False):
         fp, dp = ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)
         lib.rpy_bench_pipe_probe.restype = cint
         lib.rpy_bench_pipe_probe.argtypes = [cint, cint, vp, fp, dp, vp]
+        lib.rpy_bench_operand_probe.restype = cint
+        lib.rpy_bench_operand_probe.argtypes = [cint, cint, cint, vp, fp, dp, vp]
         lib.rpy_bench_coissue_probe.restype = cint
         lib.rpy_bench_coissue_probe.argtypes = [cint, cint, cint, cint, vp, fp, dp, dp, vp]
         lib.rpy_bench_matvec_phases.restype = cint
@@ -89,6 +92,26 @@ def pipe_probe(kind: int, iters: int = 4096, device=None) -> dict:
     if rc != 0:
         raise RuntimeError(f"rpy_bench_pipe_probe failed with status {rc}")
     return {"ms": ms.value, "fma": cnt.value, "gfma_per_s": cnt.value / (ms.value * 1e-3) / 1e9}
+
+
+OPERAND_FORMS = {0: "ffma2_two_pairs", 1: "ffma2_two_pairs_imm", 2: "ffma2_three_pairs", 3: "ffma2_three_pairs_one_reused",
+                 4: "ffma2_two_pairs_one_scalar", 5: "dfma_two_regs", 6: "dfma_three_regs", 7: "dfma_three_regs_one_reused"}
+
+
+def operand_probe(kind: int, ctas_per_sm: int = 4, iters: int = 8192, device=None) -> dict:
+    """Lane operations per second of an FFMA2 (kind 0-4) or DFMA (5-7) stream by operand form (OPERAND_FORMS)."""
+    import torch
+    lib = load_library()
+    device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    scratch = torch.zeros(8 + 8 * 128 * 4 * 12, dtype=torch.uint8, device=device)
+    ms, cnt = ctypes.c_float(), ctypes.c_double()
+    with torch.cuda.device(device):
+        stream = torch.cuda.current_stream(device).cuda_stream
+        rc = lib.rpy_bench_operand_probe(int(kind), int(ctas_per_sm), int(iters), scratch.data_ptr(), ctypes.byref(ms),
+                                         ctypes.byref(cnt), stream)
+    if rc != 0:
+        raise RuntimeError(f"rpy_bench_operand_probe failed with status {rc}")
+    return {"form": OPERAND_FORMS[int(kind)], "ms": ms.value, "tlaneops_per_s": cnt.value / (ms.value * 1e-3) / 1e12}
 
 
 def coissue_probe(n64_per_sm: int, iters32: int, iters64: int, three_reg: bool = False, device=None) -> dict:

@@ -104,6 +104,64 @@ __global__ void __launch_bounds__(kThreads) probe_kernel(int iters, float seed, 
     }
 }
 
+// ---- cost of an FP-pipe instruction by operand form (rpy_bench_operand_probe)
+// 12 independent accumulators per thread, 128 threads per CTA, `ctas_per_sm` CTAs per SM (the symmetric kernel runs 3
+// (fp32) / 4 (fp64) such CTAs per SM).  Operands come from device memory as 64-bit loads so that every packed value sits
+// in an aligned register pair (values built from scalars make the compiler insert MOVs into the loop).
+constexpr int kFormChains = 12;
+
+template <int KIND>
+__global__ void __launch_bounds__(128, 4) form_kernel(int iters, const double* __restrict__ in, double* sink)
+{
+    constexpr int NC = kFormChains;
+    if (KIND < 5) {
+        const float2* in2 = reinterpret_cast<const float2*>(in);
+        float2 acc[NC], x[NC], y[NC];
+        float sc[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            acc[c] = in2[(3 * c + 0) * 128 + threadIdx.x];
+            x[c] = in2[(3 * c + 1) * 128 + threadIdx.x];
+            y[c] = in2[(3 * c + 2) * 128 + threadIdx.x];
+            sc[c] = in2[(3 * NC + c) * 128 + threadIdx.x].x;
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                if (KIND == 0) acc[c] = __ffma2_rn(x[c], x[c], acc[c]);                        // two distinct register pairs
+                if (KIND == 1) acc[c] = __ffma2_rn(x[c], make_float2(1.5f, 1.5f), acc[c]);     // two pairs and an immediate
+                if (KIND == 2) acc[c] = __ffma2_rn(x[c], y[(c + 5) % NC], acc[c]);             // three distinct pairs, none shared with the neighbours
+                if (KIND == 3) acc[c] = __ffma2_rn(x[c], y[0], acc[c]);                        // three distinct pairs, one the same as the neighbour's (.reuse)
+                if (KIND == 4) acc[c] = __ffma2_rn(x[c], make_float2(sc[c], sc[c]), acc[c]);   // two pairs and one 32-bit scalar (.F32 operand)
+            }
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) s += acc[c].x + acc[c].y;
+        if (s == 12345.678f) sink[0] = s;
+    } else {
+        double acc[NC], x[NC], y[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            acc[c] = in[(3 * c + 0) * 128 + threadIdx.x];
+            x[c] = in[(3 * c + 1) * 128 + threadIdx.x];
+            y[c] = in[(3 * c + 2) * 128 + threadIdx.x];
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                if (KIND == 5) acc[c] = fma(x[c], x[c], acc[c]);
+                if (KIND == 6) acc[c] = fma(x[c], y[(c + 5) % NC], acc[c]);
+                if (KIND == 7) acc[c] = fma(x[c], y[0], acc[c]);
+            }
+        }
+        double s = 0.;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) s += acc[c];
+        if (s == 12345.678) sink[0] = s;
+    }
+}
+
 // ---- FP64 pipe beside the FP32 pipe
 constexpr int kMixChains = 12;
 constexpr int kMixThreads = 128;
@@ -240,5 +298,44 @@ extern "C" int rpy_bench_pipe_probe(int kind, int iters, void* d_sink, float* h_
     *h_elapsed_ms = ms;
     double per_thread = (double)iters * kChains * ((kind == 1 || kind == 4) ? 2.0 : 1.0);
     *h_fma_count = per_thread * kThreads * (double)grid.x;
+    return 0;
+}
+
+extern "C" int rpy_bench_operand_probe(int kind, int ctas_per_sm, int iters, void* d_scratch, float* h_elapsed_ms,
+                                       double* h_lane_ops, void* cuda_stream)
+{
+    if (kind < 0 || kind > 7 || iters < 1 || ctas_per_sm < 1 || ctas_per_sm > 4) return 2;
+    if (!d_scratch || !h_elapsed_ms || !h_lane_ops) return 1;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return 5;
+    dim3 grid(kNumSMs * ctas_per_sm);
+    const double* in = static_cast<const double*>(d_scratch) + 1;      // [0] is the sink
+    double* sink = static_cast<double*>(d_scratch);
+    auto launch = [&](int n) {
+        switch (kind) {
+            case 0: form_kernel<0><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 1: form_kernel<1><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 2: form_kernel<2><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 3: form_kernel<3><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 4: form_kernel<4><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 5: form_kernel<5><<<grid, 128, 0, st>>>(n, in, sink); break;
+            case 6: form_kernel<6><<<grid, 128, 0, st>>>(n, in, sink); break;
+            default: form_kernel<7><<<grid, 128, 0, st>>>(n, in, sink); break;
+        }
+    };
+    launch(iters > 64 ? 64 : iters);
+    cudaEventRecord(e0, st);
+    launch(iters);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess) return 5;
+    *h_elapsed_ms = ms;
+    *h_lane_ops = (double)iters * kFormChains * (kind < 5 ? 2.0 : 1.0) * 128.0 * (double)grid.x;
     return 0;
 }

@@ -21,6 +21,20 @@ extern "C" {
 int rpy_bench_pipe_probe(int kind, int iters, void *d_sink, float *h_elapsed_ms, double *h_fma_count,
                          void *cuda_stream);
 
+/* What an FP-pipe instruction costs by the form of its operands (the all-pairs kernels are bound
+ * by the delivery of register operands, not by the pipe itself).  12 independent accumulators per thread, 128 threads per
+ * CTA, `ctas_per_sm` (1..4) CTAs per SM; operands are loaded once from d_scratch (zeros) as 64-bit words.
+ *   kind 0 FFMA2 acc = x*x + acc          two distinct register pairs
+ *        1 FFMA2 acc = x*1.5 + acc        two pairs and an immediate
+ *        2 FFMA2 acc = x*y' + acc         three distinct pairs, none shared with the neighbouring instructions
+ *        3 FFMA2 acc = x*y0 + acc         three distinct pairs, one the same for all (served by the operand-reuse cache)
+ *        4 FFMA2 acc = x*s + acc          two pairs and a 32-bit scalar operand (.F32 broadcast form)
+ *        5, 6, 7 DFMA                     as 0, 2, 3
+ * d_scratch: >= 8 + 8 * 128 * 4 * 12 bytes of zeroed device memory.  *h_lane_ops: scalar (lane) operations executed.
+ * Returns 0, or 1 (NULL pointer), 2 (bad argument), 5 (CUDA error).                                               */
+int rpy_bench_operand_probe(int kind, int ctas_per_sm, int iters, void *d_scratch, float *h_elapsed_ms,
+                            double *h_lane_ops, void *cuda_stream);
+
 /* FP64 pipe beside the FP32 pipe: 8 CTAs of 128 threads per SM, of which `n64_per_sm` (0..8) run DFMA
  * chains of `iters64` steps and the others FFMA2 chains of `iters32` steps (role by arrival order on
  * the SM).  three_reg != 0: three distinct register operands per instruction.  Outputs: duration and

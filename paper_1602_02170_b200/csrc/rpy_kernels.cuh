@@ -435,9 +435,9 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
 #pragma unroll
                 for (int t = 0; t < T; ++t) {
                     pair_post<L, WALL>(zi2[t], zj, pre[t], c[t]);
-                    pair_apply<L, WALL>(c[t], lj0, lj1, lj2, acc[t][0], acc[t][1], acc[t][2]);
-                    if constexpr (WALL) { V tmp = c[t].ga; c[t].ga = c[t].ep; c[t].ep = tmp; }   // M^T: xz <-> zx
-                    pair_apply<L, WALL>(c[t], lt[t][0], lt[t][1], lt[t][2], uj[0], uj[1], uj[2]);
+                    // forward (u_i += M_ij lambda_j) and transposed (u_j += M_ij^T lambda_i) side by side
+                    pair_apply_both<L, WALL>(c[t], lj0, lj1, lj2, acc[t][0], acc[t][1], acc[t][2],
+                                             lt[t][0], lt[t][1], lt[t][2], uj[0], uj[1], uj[2]);
                 }
                 const int from = (lane + 1) & 31;              // the lane that just served group g + 1
                 uj[0] = shfl_from<V>(uj[0], from);

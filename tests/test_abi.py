@@ -182,7 +182,7 @@ def test_bench_aids_are_a_library_of_their_own():
     lib = bench_aids.load_library()
     hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "bench_aids", "rpy_bench_aids.h")).read(), flags=re.S)
     names = sorted(set(re.findall(r"\b(rpy_bench_[a-z0-9_]+)\s*\(", hdr)))
-    assert names == ["rpy_bench_coissue_probe", "rpy_bench_matvec_phases", "rpy_bench_pipe_probe"]
+    assert names == ["rpy_bench_coissue_probe", "rpy_bench_matvec_phases", "rpy_bench_operand_probe", "rpy_bench_pipe_probe"]
     for n in names:
         assert hasattr(lib, n)
     product = binding.load_library()
@@ -194,6 +194,9 @@ def test_bench_aids_are_a_library_of_their_own():
     assert lib.rpy_bench_pipe_probe(9, 10, one, None, None, None) == 2
     assert lib.rpy_bench_pipe_probe(0, 10, None, None, None, None) == 1
     assert lib.rpy_bench_coissue_probe(9, 10, 10, 0, one, None, None, None, None) == 2
+    assert lib.rpy_bench_operand_probe(8, 4, 10, one, None, None, None) == 2
+    assert lib.rpy_bench_operand_probe(0, 5, 10, one, None, None, None) == 2
+    assert lib.rpy_bench_operand_probe(0, 4, 10, None, None, None, None) == 1
     assert lib.rpy_bench_matvec_phases(1, 0, 10, 1, one, one, one, 1.0, 1.0, one, 1 << 20, None, None) == 1
 
 
