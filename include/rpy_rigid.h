@@ -53,11 +53,14 @@ extern "C" {
 #define RPY_ERR_NOT_SPD 6
 
 /* Third value of matvec_prec accepted by the solve only: fp32 products inside every GMRES cycle, an
- * fp64 product for the residual each cycle starts from.  "Krylov methods ... allow one to lower the
- * accuracy of the matrix-vector product as the residual is reduced": a cycle ends
- * when its fp32 residual estimate has dropped by 1e-4 (or reached tol), x is updated, the true fp64
- * residual of Eq. (11) is recomputed and decides convergence (tol = 1e-8: two cycles, two fp64 products).  Reaches fp64 tolerances at mostly
- * fp32 cost; *h_rel_resid is then the TRUE relative residual. */
+ * fp64 product for the residual a later cycle starts from.  "Krylov methods ... allow one to lower the
+ * accuracy of the matrix-vector product as the residual is reduced": a cycle that starts
+ * from the TRUE residual rho ends with a true residual within margin = 1e-5 * rho of its Arnoldi estimate
+ * (1e-5: the tolerance of the fp32 product).  While margin > tol / 2 a cycle ends when its estimate has
+ * dropped by 1e-4, x is updated and the fp64 residual of Eq. (11) is recomputed; once margin <= tol / 2 the
+ * cycle runs until estimate <= tol - margin and the solve returns without another fp64 product
+ * (tol = 1e-8: two cycles, ONE fp64 product).  *h_rel_resid is then estimate + margin, an upper bound of
+ * the true relative residual; when the solve stops after an fp64 residual (max_iter) it is that residual. */
 #define RPY_PREC_MIXED 2
 
 /* out[i] = beta * out[i] + alpha * (K U)_i.   beta == 0 overwrites (out may be uninitialised).
