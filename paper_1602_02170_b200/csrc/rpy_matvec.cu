@@ -23,6 +23,7 @@ thread_local int g_last_cuda_error = 0;
 constexpr int kAbiVersion = 5;
 constexpr int kNumSMs = 148;             // B200: 2 dies x 74 SMs
 constexpr int kTargetCtas = kNumSMs * 64;  // no source chunking beyond this many CTAs
+constexpr int kSymTargetCtas = kNumSMs * 256;   // the symmetric kernel's chunks of tile distances aim at this many
 constexpr int kMaxChunks = 64;
 constexpr int kBlock = 128;
 constexpr int kMaxT = 2;
@@ -128,7 +129,7 @@ size_t partial_bytes_bound(rpy_prec prec, int64_t n, int K, int64_t rows)
 {
     int ts = tile_sources_of(prec);
     int64_t n_tiles = (n + ts - 1) / ts;
-    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + 2 * rows;   // symmetric path: chunks + 1 slices
+    int64_t a = (int64_t)kTargetCtas * kBlock * (K <= 2 ? kMaxT : 1) + 2 * rows;   // (the symmetric path needs one slice)
     int64_t b = n_tiles * rows;
     return align_up((size_t)(a < b ? a : b) * (size_t)K * 3 * sizeof(double), kAlign);
 }
@@ -217,7 +218,9 @@ SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
     p.d_end = (int)((int64_t)all * (sh.index + 1) / sh.count);
     int count = p.d_end - p.d_begin;
     if (count < 1) count = 1;                                  // an empty shard still launches (and writes zeros)
-    int64_t want = (kTargetCtas + p.nt - 1) / p.nt;
+    // many short CTAs: measured (cfg 3 / cfg 4, fp32, G pairs/s) 148 x 64 CTAs 914.6 / 909.9, x 128 915.3 / 918.3,
+    // x 256 918.7 / 921.8, x 512 920.1 / 921.8
+    int64_t want = (kSymTargetCtas + p.nt - 1) / p.nt;
     if (want > count) want = count;
     if (want < 1) want = 1;
     p.d_per_chunk = (int)((count + want - 1) / want);

@@ -85,9 +85,9 @@ def test_launch_plan_covers_all_sources_and_fits_workspace(prec, n, k):
             d_per_chunk = -(-count // nch)
             assert d_per_chunk * nch >= count and d_per_chunk * (nch - 1) < count
             assert p["n_ctas"] == nt * nch
-            # records padded to whole tiles + (chunks + 1) slices of double partials (the extra
-            # slice takes the transposed half)
-            need = (nt * ts // w) * rec + (nch + 1) * n * 3 * 8
+            # records padded to whole tiles + the ONE double accumulator that receives both halves of every CTA's
+            # work through fp64 atomics
+            need = (nt * ts // w) * rec + n * 3 * 8
         else:
             n_tiles = -(-n // ts)
             assert 1 <= nch <= max(1, n_tiles)
