@@ -55,10 +55,11 @@ extern "C" {
 /* Third value of matvec_prec accepted by the solve only: fp32 products inside every GMRES cycle, an
  * fp64 product for the residual a later cycle starts from.  "Krylov methods ... allow one to lower the
  * accuracy of the matrix-vector product as the residual is reduced": a cycle that starts
- * from the TRUE residual rho ends with a true residual within margin = 1e-5 * rho of its Arnoldi estimate
- * (1e-5: the tolerance of the fp32 product).  While margin > tol / 2 a cycle ends when its estimate has
- * dropped by 1e-4, x is updated and the fp64 residual of Eq. (11) is recomputed; once margin <= tol / 2 the
- * cycle runs until estimate <= tol - margin and the solve returns without another fp64 product
+ * from the TRUE residual rho ends with a true residual within margin = 1e-4 * rho of its Arnoldi estimate
+ * (the fp32 product's error on the cycle's correction: a few eps_fp32 x cond(M); measured 0.3e-5 .. 2.2e-5).
+ * While margin > tol / 2 a cycle ends when its estimate has dropped by 1e-4 (or to tol / 2e-4, from where the
+ * next cycle can finish), x is updated and the fp64 residual of Eq. (11) is recomputed; once margin <= tol / 2
+ * the cycle runs until estimate <= tol - margin and the solve returns without another fp64 product
  * (tol = 1e-8: two cycles, ONE fp64 product).  *h_rel_resid is then estimate + margin, an upper bound of
  * the true relative residual; when the solve stops after an fp64 residual (max_iter) it is that residual. */
 #define RPY_PREC_MIXED 2

@@ -245,9 +245,9 @@ def test_mixed_precision_solve_reaches_fp64_tolerance_with_fp32_products():
     true_res = np.linalg.norm(res) / np.sqrt(np.sum(slip ** 2) + np.sum(b.F ** 2))
     assert true_res <= 1.001e-9
     # reading A21: the last cycle is not confirmed by an fp64 product; what is reported is its estimate plus the margin
-    # of the fp32 products (1e-5 x the true residual the cycle started from) -- an upper bound of the true residual
+    # of the fp32 products (1e-4 x the true residual the cycle started from) -- an upper bound of the true residual
     assert true_res <= r["rel_resid"] * (1 + 1e-9), (true_res, r["rel_resid"])
-    assert r["rel_resid"] - true_res <= 1e-5 * 1e-3, (true_res, r["rel_resid"])      # and a tight one
+    assert r["rel_resid"] - true_res <= 0.5 * 1e-9, (true_res, r["rel_resid"])       # margin <= tol / 2
     full = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=1e-9)
     print(f"mixed: {r['n_iter']} fp32 iterations; fp64: {full['n_iter']} iterations")
     assert r["n_iter"] <= 2 * full["n_iter"] + 4
