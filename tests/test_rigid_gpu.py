@@ -253,6 +253,24 @@ def test_mixed_precision_solve_reaches_fp64_tolerance_with_fp32_products():
     assert r["n_iter"] <= 2 * full["n_iter"] + 4
 
 
+@pytest.mark.parametrize("tol", [1e-4, 1e-6, 1e-8, 1e-10])
+def test_mixed_solve_reports_an_upper_bound_of_the_true_residual(tol):
+    """Reading A21 on config 2 (1,000 boomerangs, N = 15,000): whatever the tolerance -- one cycle confirmed by the fp64
+    residual (1e-4), two cycles of which the last is not confirmed (1e-6, 1e-8) or three (1e-10) -- the residual
+    re-evaluated with the fp64 operator is below what the solve reports, and that is below tol."""
+    w = workloads.make(2)
+    b = workloads.bodies_of(w)
+    db = rigid.bodies(dev(w.pos), dev(b.q), b.offsets)
+    slip = 0.1 * np.random.default_rng(8).standard_normal(w.pos.shape)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    r = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=tol, matvec_prec="mixed")
+    x = torch.cat([r["lambda"].reshape(-1), r["U"].reshape(-1)])
+    res = rigid.rpy_rigid_saddle_apply(db, x, "wall").cpu().numpy() - np.concatenate([slip.ravel(), -b.F.ravel()])
+    true_res = np.linalg.norm(res) / np.sqrt(np.sum(slip ** 2) + np.sum(b.F ** 2))
+    print(f"mixed, tol {tol:g}: {r['n_iter']} iterations, reported {r['rel_resid']:.3e}, true {true_res:.3e}")
+    assert true_res <= r["rel_resid"] * (1 + 1e-9) <= tol * (1 + 1e-9)
+
+
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("mixed", 1e-9), ("f32", 1e-5)])
 def test_batched_solve_equals_the_single_solves_and_the_dense_oracle(prec, tol):
     """k right-hand sides in lockstep (one k-right-hand-side product per iteration): every right-hand side
