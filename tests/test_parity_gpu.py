@@ -187,6 +187,35 @@ def test_single_blob_and_coincident_blobs(prec):
         check(u, ref, prec, f"coincident/r=2a {variant}")
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [700, 4000])
+def test_dense_cluster_where_most_pairs_overlap(prec, n):
+    """The r <= 2a branch of Eq. (9) is rare in the configured workloads (it sits behind a warp vote); here it is the rule:
+    blobs packed into a box 3a wide (every pair overlaps) or 12a wide (most warp steps take the vote), plain kernel (n = 700)
+    and symmetric kernel (n = 4,000); two blobs coincide."""
+    rng = np.random.default_rng(31)
+    side = 3.0 if n == 700 else 12.0
+    pos = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(1.1, 1.1 + side, n)])
+    pos[n // 2] = pos[n // 3]
+    lam = rng.standard_normal((1, n, 3))
+    for variant in ("wall", "free"):
+        u, ref = run_case(pos, lam, prec, variant)
+        check(u, ref, prec, f"dense cluster n={n} {variant}")
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_blobs_overlapping_the_wall_formula_as_is(prec):
+    """Reading A6: for z < a the tensor is not meaningful but it is evaluated as written, with no
+    clamping inside the library: blobs at heights 0.3a .. a (and some below 0.05a) give the oracle's numbers."""
+    rng = np.random.default_rng(32)
+    n = 900
+    pos = np.column_stack([rng.uniform(0, 40, n), rng.uniform(0, 40, n), rng.uniform(0.3, 1.0, n)])
+    pos[:20, 2] = rng.uniform(0.01, 0.05, 20)
+    lam = rng.standard_normal((2, n, 3))
+    u, ref = run_case(pos, lam, prec, "wall")
+    check(u, ref, prec, "blobs overlapping the wall")
+
+
 def test_empty_and_zero_force():
     e = torch.zeros(0, 3, dtype=torch.float64, device="cuda")
     assert binding.rpy_wall_matvec(e, e).shape == (0, 3)
