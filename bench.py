@@ -428,7 +428,7 @@ def size_sweep(torch):
     from paper_1602_02170_b200 import binding, workloads
     lane = {"f32": SM_COUNT * LANES["f32"] * SM_MAX_GHZ * 1e9, "f64": SM_COUNT * LANES["f64"] * SM_MAX_GHZ * 1e9}
     rows = []
-    for n in (1000, 2000, 3000, 3584, 4000, 6144, 8000, 10000, 15000, 20000, 30000, 50000, 100000, 172032):
+    for n in (1000, 1152, 1500, 2000, 3000, 3584, 4000, 6144, 8000, 10000, 15000, 20000, 30000, 50000, 100000, 172032):
         w = workloads.config1(seed=0, n=n)
         for prec, dt in (("f32", torch.float32), ("f64", torch.float64)):
             pos = torch.from_numpy(w.pos).to(dt).cuda(); lam = torch.from_numpy(w.force).to(dt).cuda()

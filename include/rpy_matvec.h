@@ -113,7 +113,7 @@ rpy_status rpy_free_matvec_rows(rpy_prec prec, int64_t n_blobs, int n_rhs,
  * 3 n_rhs n_blobs doubles).  d_vel [n_rhs][n_blobs][3] is overwritten with the shard's contribution
  * to EVERY row and is DOUBLE on both paths: the cross-shard sum is part of the "fp64 accumulation" of
  * the fp32 path and must not round to float per shard (pos and force keep the path's type).
- * For n_rhs == 1 and n_blobs >= 3,584 a shard is a contiguous range of the tile
+ * For n_rhs == 1 and n_blobs >= 1,152 a shard is a contiguous range of the tile
  * distances of the symmetric kernel (all distances cost the same, so shards are balanced); otherwise
  * it is a contiguous range of target rows of the plain kernel and the other rows are zero.
  * 0 <= shard < n_shards <= 4096.  Workspace: rpy_matvec_workspace_bytes().                        */
@@ -182,7 +182,7 @@ rpy_status rpy_wall_count_below(rpy_prec prec, int64_t n_blobs, const void *d_po
  * Pure host arithmetic (no CUDA call); any output pointer may be NULL.
  *   *symmetric == 0: the plain kernel.  A CTA owns *targets_per_cta target rows and walks one of
  *     *n_source_chunks contiguous chunks of the sources in shared-memory tiles of *tile_sources.
- *   *symmetric == 1: the symmetric kernel (n_rhs == 1, all rows, n_blobs >= 3,584), which uses
+ *   *symmetric == 1: the symmetric kernel (n_rhs == 1, all rows, n_blobs >= 1,152), which uses
  *     M_ij = M_ji^T to build every unordered pair's coefficients once.  Blobs are
  *     cut into tiles of *tile_sources (= *targets_per_cta: 128 below 50,000 blobs, else 256); a CTA owns one tile I and walks the
  *     tiles (I + d) mod n_tiles for one of *n_source_chunks chunks of the distances d = 0..n_tiles/2.

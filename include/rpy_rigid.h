@@ -143,7 +143,7 @@ size_t rpy_rigid_solve_workspace_bytes(rpy_prec matvec_prec, int64_t n_blobs, in
  *       tile pairs) and calls reduce(reduce_ctx, d_buf, count, cuda_stream) once per product; the hook must
  *       make d_buf[0..count) (doubles, device) the SUM over all ranks, in stream order on cuda_stream (e.g.
  *       an in-place NCCL all-reduce), and return 0.  Everything else of the iteration is replicated, so the
- *       ranks take the same decisions.  n_shards > 1 needs n_rhs == 1 and n_blobs >= 3,584.              */
+ *       ranks take the same decisions.  n_shards > 1 needs n_rhs == 1 and n_blobs >= 1,152.              */
 typedef int (*rpy_reduce_fn)(void *reduce_ctx, double *d_buf, int64_t count, void *cuda_stream);
 typedef struct rpy_rigid_solve_ext {
     void *side_stream;

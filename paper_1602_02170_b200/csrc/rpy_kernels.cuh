@@ -320,7 +320,7 @@ template <> __device__ __forceinline__ double lane_elem<float2>(float2 v, int w)
 template <class L, bool WALL, int T, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ gacc,
-                    int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end,
+                    int64_t n_blobs, int nt, int d_per_chunk, int d_begin, int d_end, int split,
                     const int* __restrict__ skip)
 {
     using V = typename L::V;
@@ -337,6 +337,13 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     constexpr int kUnroll = IS_F64 ? RPY_SYM_UNROLL_F64 : RPY_SYM_UNROLL_F32;
     constexpr uint32_t TILE_BYTES = (uint32_t)TILE_G * R::BYTES;
     static_assert(TILE_G % 32 == 0 && R::LEN * sizeof(S) == 48, "record geometry");
+    // Small problems do not fill the chip with one CTA per tile pair (N = 2,000: 136 tile pairs of 128 blobs for 888
+    // resident CTAs): the host may cut every tile pair into `split` parts (grid z); this CTA then meets only the sub-tiles
+    // p_lo .. p_lo + cnt - 1 of each tile J (and stages only those), with all of its own targets.
+    const int cnt = NSUB / split;                  // sub-tiles per tile for this CTA (split divides NSUB)
+    const int p_lo = (int)blockIdx.z * cnt;
+    const uint32_t part_bytes = (uint32_t)cnt * 32u * R::BYTES;
+    const int64_t part_off = (int64_t)p_lo * 32 * R::BYTES;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* const buf0 = smem_raw;
@@ -363,8 +370,8 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
     const unsigned char* gbase = reinterpret_cast<const unsigned char*>(rec);
     auto tile_of = [&](int it) { int J = I + d_lo + it; return J >= nt ? J - nt : J; };
     if (tid == 0 && my_tiles > 0) {
-        mbar_expect_tx(&full_bar[0], TILE_BYTES);
-        bulk_g2s(buf0, gbase + (int64_t)tile_of(0) * TILE_BYTES, TILE_BYTES, &full_bar[0]);
+        mbar_expect_tx(&full_bar[0], part_bytes);
+        bulk_g2s(buf0, gbase + (int64_t)tile_of(0) * TILE_BYTES + part_off, part_bytes, &full_bar[0]);
     }
 
     V xi[T], yi[T], zi[T], zi2[T], li[T][3];
@@ -396,11 +403,11 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
         const int b = it & 1;
         __syncthreads();                                       // buffer b^1 is free again
         if (tid == 0 && it + 1 < my_tiles) {
-            mbar_expect_tx(&full_bar[b ^ 1], TILE_BYTES);
-            bulk_g2s(buf0 + (b ^ 1) * TILE_BYTES, gbase + (int64_t)tile_of(it + 1) * TILE_BYTES, TILE_BYTES, &full_bar[b ^ 1]);
+            mbar_expect_tx(&full_bar[b ^ 1], part_bytes);
+            bulk_g2s(buf0 + (b ^ 1) * TILE_BYTES, gbase + (int64_t)tile_of(it + 1) * TILE_BYTES + part_off, part_bytes, &full_bar[b ^ 1]);
         }
         mbar_wait(&full_bar[b], (uint32_t)((it >> 1) & 1));
-        const S* tile = reinterpret_cast<const S*>(buf0 + b * TILE_BYTES);
+        const S* tile = reinterpret_cast<const S*>(buf0 + b * TILE_BYTES);     // holds sub-tiles p_lo .. p_lo + cnt - 1 of J
         const int J = tile_of(it);
         const bool diagonal = (d_lo + it) == 0;
         V lt[T][3];                                            // lambda_i as seen by the transposed application
@@ -410,9 +417,12 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
             for (int c = 0; c < 3; ++c) lt[t][c] = diagonal ? L::bc(0.0) : li[t][c];
 
 #pragma unroll 1
-        for (int p = 0; p < NSUB; ++p) {
-            const int q = (p + warp * (NSUB / NWARP > 0 ? NSUB / NWARP : 1)) % NSUB;
-            const S* sub = tile + (q * 32) * R::LEN;
+        for (int p = 0; p < cnt; ++p) {
+            // the warps start on different sub-tiles (when the CTA has several) so that they do not flush the same
+            // addresses together; ql = index inside the staged part, q = index inside the tile
+            const int ql = (p + warp * (NSUB / NWARP > 0 ? NSUB / NWARP : 1)) % cnt;
+            const int q = p_lo + ql;
+            const S* sub = tile + (ql * 32) * R::LEN;
             V uj[3] = {L::bc(0.0), L::bc(0.0), L::bc(0.0)};
 #pragma unroll kUnroll              // measured (cfg 3): fp32 881 / 897 / 899 G pairs/s with 2 / 4 / 8; fp64 374 / 381 / 387 with 1 / 2 / 4
             for (int s = 0; s < 32; ++s) {

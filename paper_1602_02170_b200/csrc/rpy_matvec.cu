@@ -30,7 +30,7 @@ constexpr int kMaxT = 2;
 constexpr size_t kAlign = 256;
 constexpr int kSymTile = kBlock * 2;       // blobs per tile of the symmetric kernel (T = 2)
 #ifndef RPY_SYM_MIN_BLOBS
-#define RPY_SYM_MIN_BLOBS 3584
+#define RPY_SYM_MIN_BLOBS 1152
 #endif
 constexpr int64_t kSymMinBlobs = RPY_SYM_MIN_BLOBS;   // below this the plain kernel is used (too few tile pairs to fill the chip)
 
@@ -180,8 +180,11 @@ cudaError_t launch_allpairs(const Plan& p, const typename L::S* rec, const typen
 }
 
 // Symmetric path (rpy::allpairs_sym_kernel): one right-hand side, all rows, enough tiles.
-struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_begin; int d_end; int tile; };
+struct SymPlan { int nt; int d_per_chunk; int n_chunks; int64_t n_padded; int d_begin; int d_end; int tile; int split; };
 
+#ifndef RPY_SYM_SPLIT_BELOW_CTAS_PER_SM
+#define RPY_SYM_SPLIT_BELOW_CTAS_PER_SM 6
+#endif
 #ifndef RPY_SYM_SMALL_BELOW
 #define RPY_SYM_SMALL_BELOW 50000      // below this many blobs the symmetric kernel runs with 128-blob tiles (measured crossover)
 #endif
@@ -204,7 +207,8 @@ inline bool use_symmetric(int64_t n, int K, int64_t row_begin, int64_t rows)
     return K == 1 && row_begin == 0 && rows == n && n >= kSymMinBlobs;
 }
 
-SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
+// max_split: 32-record sub-tiles of a 128-blob tile (2 with two blobs per record, 4 with one)
+SymPlan make_sym_plan(int64_t n, int max_split, Shard sh = Shard{0, 1})
 {
     SymPlan p;
     // Tiles of 256 blobs (128 threads x 2 targets) once there are enough of them to fill the chip several
@@ -225,6 +229,15 @@ SymPlan make_sym_plan(int64_t n, Shard sh = Shard{0, 1})
     if (want < 1) want = 1;
     p.d_per_chunk = (int)((count + want - 1) / want);
     p.n_chunks = (count + p.d_per_chunk - 1) / p.d_per_chunk;
+    // Small problems: one CTA per tile pair does not fill the chip (N = 2,000: 136 tile pairs for 148 x 6 resident CTAs of
+    // 64 threads): cut every tile pair into two halves of its source tile (grid z).  Past that point the halves only add
+    // set-up and flush work (measured: N = 3,584 29.2 -> 24.0 us, N >= 4,000 within 2 %).
+    p.split = 1;
+#ifndef RPY_SYM_NO_SPLIT
+    if (p.tile == kSymTile / 2 && p.d_per_chunk == 1)
+        while (p.split < max_split && (int64_t)p.nt * p.n_chunks * p.split <= (int64_t)kNumSMs * RPY_SYM_SPLIT_BELOW_CTAS_PER_SM)
+            p.split *= 2;
+#endif
     return p;
 }
 
@@ -237,20 +250,20 @@ cudaError_t launch_sym(bool wall, const SymPlan& p, const typename L::S* rec, do
                        int64_t n, cudaStream_t st, const int* skip)
 {
     constexpr int MINB = SymShape<L>::MINB;
-    dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks);
+    dim3 grid((unsigned)p.nt, (unsigned)p.n_chunks, (unsigned)p.split);
     if (p.tile == kSymTile) {
         size_t smem = 2 * (size_t)(kSymTile / L::W) * rpy::RecLayout<L, 1>::BYTES;
         if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
-                                         rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                                         rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, p.split, skip);
         return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, kBlock, MINB>, grid, dim3(kBlock), smem, st,
-                               rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                               rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, p.split, skip);
     }
     constexpr int B2 = kBlock / 2;
     size_t smem = 2 * (size_t)(kSymTile / 2 / L::W) * rpy::RecLayout<L, 1>::BYTES;
     if (wall) return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, true, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
-                                     rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                                     rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, p.split, skip);
     return rpy::launch_pdl(rpy::allpairs_sym_kernel<L, false, 2, B2, 2 * MINB>, grid, dim3(B2), smem, st,
-                           rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, skip);
+                           rec, gacc, n, p.nt, p.d_per_chunk, p.d_begin, p.d_end, p.split, skip);
 }
 
 template <class L, int K>
@@ -281,7 +294,7 @@ cudaError_t run_group(bool wall, int64_t n, int64_t row_begin, int64_t rows,
     double* partial = reinterpret_cast<double*>(ws + at);
     const bool sym = !tpos && use_symmetric(n, K, row_begin, rows);
     const Plan p = make_plan(prec, n, K, rows);
-    const SymPlan sp = make_sym_plan(n, sh);
+    const SymPlan sp = make_sym_plan(n, kSymTile / 2 / L::W / 32, sh);
     const int64_t n_padded = sym ? sp.n_padded : p.n_padded;
     cudaError_t e;
     int n_slices = p.n_chunks;
@@ -701,11 +714,11 @@ rpy_status rpy_matvec_launch_plan(rpy_prec prec, int64_t n_blobs, int n_rhs, int
     if (n_blobs < 0 || n_blobs > RPY_MAX_BLOBS || n_rhs < 1 || row_count < 0 || row_count > n_blobs) return RPY_ERR_ARG;
     const int K = group_k(n_rhs);
     if (use_symmetric(n_blobs, K, 0, row_count) && n_rhs == 1) {
-        SymPlan sp = make_sym_plan(n_blobs);
+        SymPlan sp = make_sym_plan(n_blobs, prec == RPY_PREC_F64 ? 4 : 2);
         if (targets_per_cta) *targets_per_cta = sp.tile;
         if (n_source_chunks) *n_source_chunks = sp.n_chunks;
         if (tile_sources) *tile_sources = sp.tile;
-        if (n_ctas) *n_ctas = (int64_t)sp.nt * sp.n_chunks;
+        if (n_ctas) *n_ctas = (int64_t)sp.nt * sp.n_chunks * sp.split;
         if (symmetric) *symmetric = 1;
         return RPY_OK;
     }

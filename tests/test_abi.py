@@ -78,13 +78,13 @@ def test_launch_plan_covers_all_sources_and_fits_workspace(prec, n, k):
         if p["symmetric"]:
             # symmetric kernel: one RHS, all rows, tiles of 128 (n < 50,000) or 256 blobs, chunks of the
             # tile distances 0..nt/2
-            assert k == 1 and rows == n and n >= 3584 and ts == tpc == (128 if n < 50000 else 256)
+            assert k == 1 and rows == n and n >= 1152 and ts == tpc == (128 if n < 50000 else 256)
             nt = -(-n // ts)
             count = nt // 2 + 1
             assert 1 <= nch <= count
             d_per_chunk = -(-count // nch)
             assert d_per_chunk * nch >= count and d_per_chunk * (nch - 1) < count
-            assert p["n_ctas"] == nt * nch
+            assert p["n_ctas"] in (nt * nch, 2 * nt * nch, 4 * nt * nch)       # small problems: tile pairs cut in 2 or 4
             # records padded to whole tiles + the ONE double accumulator that receives both halves of every CTA's
             # work through fp64 atomics
             need = (nt * ts // w) * rec + n * 3 * 8

@@ -100,7 +100,7 @@ def test_reproducible_paths_are_bit_identical_whatever_was_in_the_workspace(prec
     product: bit-identical across runs whose workspaces start as NaN, as zeros and as the previous run's
     leftovers.  A race on the shared-memory staging, or a read of stale workspace, would show here."""
     dt = torch.float64 if prec == "f64" else torch.float32
-    w = workloads.config2(seed=7, n_bodies=120, k=2)           # 1,800 blobs: plain kernel
+    w = workloads.config2(seed=7, n_bodies=70, k=2)            # 1,050 blobs (< 1,152): the plain kernel also inside the solve
     hb = workloads.bodies_of(w)
     pos, lam = torch.from_numpy(w.pos).to(dt).cuda(), torch.from_numpy(w.force).to(dt).cuda()
     pos64 = torch.from_numpy(w.pos).cuda()
@@ -108,7 +108,7 @@ def test_reproducible_paths_are_bit_identical_whatever_was_in_the_workspace(prec
     for rep, poison in enumerate((0xFF, 0x00, 0x7F, 0xFF)):
         with guarded(poison) as g:
             u = binding.rpy_wall_matvec(pos, lam)
-            ur = binding.rpy_free_matvec(pos, lam, rows=(100, 999))
+            ur = binding.rpy_free_matvec(pos, lam, rows=(100, 900))
             db = rigid.bodies(pos64, torch.from_numpy(hb.q).cuda(), hb.offsets)
             pc = rigid.rpy_rigid_precond_build(db, "wall")
             x = torch.arange(db.n, dtype=torch.float64, device="cuda").sin()
