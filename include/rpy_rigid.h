@@ -169,9 +169,11 @@ typedef struct rpy_rigid_solve_ext {
  *   d_F         [n_bodies][6] device;  d_slip [n_blobs][3] device or NULL (zero slip)
  *   d_lambda    [n_blobs][3], d_U [n_bodies][6] : device, overwritten
  *   h_history   host, max_iter+1 doubles or NULL: relative residual after each iteration, [0] = 1
- *   h_n_iter    host, matrix applications used;  h_rel_resid host, final relative residual: the true
- *               residual of Eq. (11) (fp64 product) unless matvec_prec is RPY_PREC_F64, where the Arnoldi
- *               estimate IS the residual of the operator used
+ *   h_n_iter    host, matrix applications used;  h_rel_resid host, final relative residual: with
+ *               RPY_PREC_F64 the Arnoldi estimate, which IS the residual of the operator used; with
+ *               RPY_PREC_F32_ACC64 the true residual of Eq. (11) (one fp64 product at the end); with
+ *               RPY_PREC_MIXED an upper bound of the true residual (see RPY_PREC_MIXED; a caller who wants the
+ *               residual itself applies rpy_rigid_saddle_apply to the solution)
  * Returns RPY_OK also when max_iter was reached without convergence (check *h_rel_resid).
  * A d_precond that was not built for these bodies (n_bodies, n_blobs) is RPY_ERR_ARG.                */
 rpy_status rpy_rigid_mobility_solve(int wall, rpy_prec matvec_prec, int64_t n_blobs, int64_t n_bodies,
