@@ -424,7 +424,7 @@ allpairs_sym_kernel(const typename L::S* __restrict__ rec, double* __restrict__ 
             const int q = p_lo + ql;
             const S* sub = tile + (ql * 32) * R::LEN;
             V uj[3] = {L::bc(0.0), L::bc(0.0), L::bc(0.0)};
-#pragma unroll kUnroll              // measured (cfg 3): fp32 881 / 897 / 899 G pairs/s with 2 / 4 / 8; fp64 374 / 381 / 387 with 1 / 2 / 4
+#pragma unroll kUnroll              // measured (cfg 3, end of round 2): fp32 896 / 912 / 908 G pairs/s with 2 / 4 / 8; fp64 391 / 391 / 397
             for (int s = 0; s < 32; ++s) {
                 const int g = (s + lane) & 31;
                 const V* r = reinterpret_cast<const V*>(sub + g * R::LEN);
