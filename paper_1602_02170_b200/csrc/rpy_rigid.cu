@@ -561,7 +561,13 @@ __device__ __forceinline__ bool pivot_inverse(const double (&A)[kRT][kRT], doubl
     for (int k = 0; k < 4; ++k) {
         const double d = P[k][k];
         ok = ok && d > 0.0 && isfinite(d);
-        const double inv = 1.0 / d;
+        // 1/d for a positive finite pivot: the MUFU.RCP64H seed and two Newton steps.  The four pivots of a block are
+        // inverted one after the other by ONE thread while the CTA waits, so the division's slow path was on the critical
+        // path (cfg 3 build 1.88 -> 1.75 ms; the inverse unchanged to 13 digits)
+        double inv;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(inv) : "d"(d));
+        inv = fma(inv, fma(-d, inv, 1.0), inv);
+        inv = fma(inv, fma(-d, inv, 1.0), inv);
         double w[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) w[i] = P[i][k] * inv;
