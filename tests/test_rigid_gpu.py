@@ -271,6 +271,28 @@ def test_mixed_solve_reports_an_upper_bound_of_the_true_residual(tol):
     assert true_res <= r["rel_resid"] * (1 + 1e-9) <= tol * (1 + 1e-9)
 
 
+@pytest.mark.parametrize("case,tol", [("boomerangs_seed3", 1e-8), ("shell_lattice_256", 1e-9), ("rods_phi0.3", 1e-8),
+                                      ("rods_phi0.3", 1e-10)])
+def test_mixed_solve_bound_holds_on_other_workloads(case, tol):
+    """The same check (reading A21) on other geometries: another draw of config 2, a 16 x 16 lattice of 42-blob shells,
+    the paper's 21-blob rods at packing fraction 0.3."""
+    if case == "boomerangs_seed3":
+        w = workloads.config2(seed=3); pos, b = w.pos, workloads.bodies_of(w)
+    elif case == "shell_lattice_256":
+        w = workloads.config3(side=16); pos, b = w.pos, workloads.bodies_of(w)
+    else:
+        pos, b = workloads.rods_near_wall(1000, 0.3, 0.75, seed=0)
+    db = rigid.bodies(dev(pos), dev(b.q), b.offsets)
+    slip = 0.1 * np.random.default_rng(8).standard_normal(pos.shape)
+    pc = rigid.rpy_rigid_precond_build(db, "wall")
+    r = rigid.rpy_rigid_mobility_solve(db, pc, dev(b.F), dev(slip), "wall", tol=tol, matvec_prec="mixed", max_iter=400)
+    x = torch.cat([r["lambda"].reshape(-1), r["U"].reshape(-1)])
+    res = rigid.rpy_rigid_saddle_apply(db, x, "wall").cpu().numpy() - np.concatenate([slip.ravel(), -b.F.ravel()])
+    true_res = np.linalg.norm(res) / np.sqrt(np.sum(slip ** 2) + np.sum(b.F ** 2))
+    print(f"{case}, tol {tol:g}: {r['n_iter']} iterations, reported {r['rel_resid']:.3e}, true {true_res:.3e}")
+    assert true_res <= r["rel_resid"] * (1 + 1e-9) <= tol * (1 + 1e-9)
+
+
 @pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("mixed", 1e-9), ("f32", 1e-5)])
 def test_batched_solve_equals_the_single_solves_and_the_dense_oracle(prec, tol):
     """k right-hand sides in lockstep (one k-right-hand-side product per iteration): every right-hand side
